@@ -1,0 +1,174 @@
+/*
+ * orb.h -- C ABI of liborb_b200: gyro-averaged charge and parallel-current
+ * deposition of delta-f markers onto a 3-D cubic B-spline grid, on one NVIDIA
+ * B200 (sm_100a).  Plain C; callers need no CUDA header.
+ *
+ * What is computed (citations are lines of arxiv 1908.02219 as extracted in
+ * PAPER.md; "R<n>" are the readings listed in DESIGN.md where the paper is
+ * silent):
+ *
+ *   rho [i,j,k] += sum_p (q w_p        / N_L(p)) sum_l Ls_i(s_pl) Lt_j(ts_pl) Lp_k(phi_p)
+ *   jpar[i,j,k] += sum_p (q w_p vpar_p / N_L(p)) sum_l Ls_i(s_pl) Lt_j(ts_pl) Lp_k(phi_p)
+ *
+ *   - markers are structure-of-arrays in magnetic coordinates (s, theta*, phi)
+ *     (PAPER.md:21, 39); fields are 3-D finite-element cubic B-splines
+ *     (PAPER.md:19, 39): clamped (open knot vector) in s, periodic in theta*, phi;
+ *   - every marker is expanded into N_L Larmor points on a ring of radius
+ *     rho_L = rho* sqrt(2 mu / B) in the poloidal plane at the marker's phi
+ *     (R5-R7), N_L fixed or proportional to the ring size
+ *     (R9);
+ *   - geometry: concentric circular flux surfaces R = R0 + a s cos(theta),
+ *     Z = a s sin(theta), B = B0 / (1 + (a/R0) s cos(theta)), theta* the
+ *     straight-field-line angle tan(theta* / 2) = sqrt((1-e)/(1+e)) tan(theta/2),
+ *     e = (a/R0) s (R1-R3);
+ *   - a point that leaves the plasma (s_l > 1) is deposited at s_l = 1 (R11);
+ *   - "deposit" without sorting loops over markers and the finite elements they
+ *     touch with atomic accumulation; with sorting, markers are
+ *     first bucket-sorted by field cell.  Both are offered here.
+ *
+ * Conventions common to all calls
+ *   - every call returns ORB_OK (0) or a negative orb_status code; nothing
+ *     throws, aborts or prints.  orb_strerror() gives a static description;
+ *     orb_last_error() the detailed message of the last failing call on a handle.
+ *   - "device pointer" = memory of the CUDA device given in the descriptor
+ *     (e.g. torch.Tensor.data_ptr()); "host pointer" = ordinary host memory.
+ *   - `stream` is a cudaStream_t passed as void* (NULL = legacy default stream).
+ *     Calls that take a stream only enqueue work on it and do not synchronise
+ *     the host, unless stated.
+ *   - there is no CPU fallback: without a usable CUDA device orb_grid_create
+ *     fails with ORB_E_CUDA.
+ */
+#ifndef ORB_H_
+#define ORB_H_
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define ORB_VERSION 100
+#define ORB_MAX_NL 32 /* largest number of Larmor points per marker */
+
+typedef enum {
+  ORB_OK = 0,
+  ORB_E_INVAL = -1, /* bad argument: NULL, n < 0, ns/ntheta/nphi < 4, a >= r0, N_L out of
+                       [1, ORB_MAX_NL], n_max < n_min, pointer not 16-byte aligned        */
+  ORB_E_STATE = -2, /* call order: deposit/bin before bind                              */
+  ORB_E_NOMEM = -3, /* scratch allocation failed                                        */
+  ORB_E_CUDA = -4   /* CUDA runtime / launch error (see orb_last_error)                 */
+} orb_status;
+
+typedef struct orb_grid orb_grid_t; /* opaque; owned by the library */
+
+/* Grid + geometry + species.  Sizes are in CELLS; the deposited arrays have
+ * (ns+3) x ntheta x nphi NODES (basis functions): the clamped cubic basis in s
+ * has ns+3 functions, the periodic ones one per cell (R11). */
+typedef struct {
+  int32_t ns, ntheta, nphi; /* >= 4 each                                                  */
+  double r0, a, b0;         /* major radius, minor radius (a < r0), field on axis (R1,R2) */
+  double rho_star;          /* thermal Larmor radius / a  (>= 0)  (R6)                    */
+  double q;                 /* species charge                                             */
+  int32_t theta_map;        /* 1: theta* is the straight-field-line angle (R3, default);
+                               0: theta* == geometric theta                               */
+  int32_t device;           /* CUDA device ordinal                                        */
+} orb_grid_desc_t;
+
+enum { ORB_NL_FIXED = 0, ORB_NL_ADAPTIVE = 1 };
+
+/* flags of orb_nl_policy_t.flags */
+#define ORB_DEPOSIT_ZERO_FIRST 0x1u  /* zero rho/jpar on the stream before adding              */
+#define ORB_DEPOSIT_NO_BIN 0x2u      /* never bin: deposit markers in the order they are bound  */
+#define ORB_DEPOSIT_ALGO_ATOMIC 0x4u /* use the one-thread-per-marker global-atomics kernel
+                                        (the GPU algorithm of) instead of the
+                                        shared-memory tile kernel                              */
+
+/* Number of Larmor points per marker (R7-R9):
+ *   FIXED:    N_L = n_fixed
+ *   ADAPTIVE: N_L = min(n_max, n_fixed * max(1, ceil(rho_L / rho_ref)))
+ * N_L = 1 deposits the guiding centre itself (R8).  Gyro-phases are
+ * alpha_l = alpha0 + 2 pi l / N_L measured from +R towards +Z. */
+typedef struct {
+  int32_t mode;    /* ORB_NL_FIXED | ORB_NL_ADAPTIVE                                      */
+  int32_t n_fixed; /* FIXED: N_L.  ADAPTIVE: n_min.   1..ORB_MAX_NL                       */
+  int32_t n_max;   /* ADAPTIVE: cap, n_fixed..ORB_MAX_NL (ignored when FIXED)             */
+  uint32_t flags;  /* ORB_DEPOSIT_*                                                       */
+  double rho_ref;  /* ADAPTIVE: reference radius in units of a (> 0)                      */
+  double alpha0;   /* gyro-phase of point 0, radians                                      */
+} orb_nl_policy_t;
+
+/* flags of orb_markers_bind */
+#define ORB_MARKERS_SORTED 0x1u /* markers are already sorted by guiding-centre cell key
+                                   (k_phi*ns + i_s)*ntheta + j_theta (non-decreasing; R17);
+                                   binning then only locates the cell boundaries            */
+
+/* Creates a handle for one grid on desc->device and allocates nothing that
+ * scales with the marker count yet.  *out is written only on success. */
+int orb_grid_create(const orb_grid_desc_t *desc, orb_grid_t **out);
+
+/* Frees the handle and all scratch.  Synchronises the device.  NULL is accepted. */
+int orb_grid_destroy(orb_grid_t *g);
+
+/* dims = (ns+3, ntheta, nphi): shape of rho / jpar, C order, k_phi fastest:
+ * index = (i_s*ntheta + j_theta)*nphi + k_phi  (R14). */
+int orb_grid_shape(const orb_grid_t *g, int64_t dims[3]);
+
+/* Binds n markers given as six DEVICE arrays of n doubles (structure of arrays,
+ * PAPER.md:21): s in [0,1], theta* and phi any finite angle in radians (wrapped to
+ * [0,2pi)), parallel velocity, magnetic moment mu >= 0, weight.  Pointers are
+ * BORROWED: no copy is made; they must stay valid and unmodified until the next
+ * bind or destroy, and the library never writes to them.  vpar may be NULL if
+ * jpar will always be NULL.  Pointers must be 16-byte aligned.  Marker VALUES are
+ * not validated.  Any previous binning is discarded.  n = 0 is legal. */
+int orb_markers_bind(orb_grid_t *g, int64_t n, const double *s, const double *theta,
+                     const double *phi, const double *vpar, const double *mu, const double *w,
+                     uint32_t flags);
+
+/* Runs (or refreshes) the binning pass alone on `stream`, so that it can be timed
+ * apart from the deposit (BASELINE.json config 4; the bucket sort of PAPER.md:167):
+ * counting sort of the bound markers by guiding-centre cell into library-owned
+ * scratch.  For ORB_MARKERS_SORTED bindings only the per-cell offsets are built.
+ * May allocate scratch on first use (which synchronises); afterwards asynchronous. */
+int orb_markers_bin(orb_grid_t *g, void *stream);
+
+/* Adds the charge density into rho and, if jpar != NULL, the parallel current
+ * into jpar (DEVICE arrays of orb_grid_shape doubles, owned by the caller).
+ * Asynchronous on `stream`.  Bins first if the markers are not binned yet, unless
+ * ORB_DEPOSIT_NO_BIN or ORB_DEPOSIT_ALGO_ATOMIC is set.  The result is the plain
+ * sum above up to fp64 summation order (atomic ordering is the only source of
+ * run-to-run difference). */
+int orb_deposit(orb_grid_t *g, double *rho, double *jpar, const orb_nl_policy_t *policy,
+                void *stream);
+
+/* Sum of N_L over the markers of the last orb_deposit on this handle.
+ * Synchronises with that deposit (one 8-byte device-to-host copy). */
+int orb_last_points(orb_grid_t *g, int64_t *n_points);
+
+/* End-to-end convenience for callers whose data lives on the HOST: copies the six
+ * marker arrays (host pointers, n doubles each; vpar may be NULL iff jpar_host is
+ * NULL) to library-owned device buffers, binds, deposits into zeroed device grids
+ * and copies rho (and jpar) back into the host arrays, which are OVERWRITTEN.
+ * Synchronous.  Leaves the handle bound to the library's own device copies.
+ * h2d_bytes / d2h_bytes (optional) receive the bytes moved. */
+int orb_deposit_host(orb_grid_t *g, int64_t n, const double *s, const double *theta,
+                     const double *phi, const double *vpar, const double *mu, const double *w,
+                     double *rho_host, double *jpar_host, const orb_nl_policy_t *policy,
+                     int64_t *n_points, int64_t *h2d_bytes, int64_t *d2h_bytes);
+
+/* Number of kernel launches the library has enqueued on this handle so far
+ * (memsets and copies not counted). */
+int orb_launch_count(const orb_grid_t *g, int64_t *n_launches);
+
+/* Static text for a status code. */
+const char *orb_strerror(int code);
+
+/* Detailed message of the last failing call on g (includes cudaGetErrorString);
+ * "" if none.  The pointer stays valid until the next call on g. */
+const char *orb_last_error(const orb_grid_t *g);
+
+int orb_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* ORB_H_ */

@@ -1,0 +1,180 @@
+"""Thin ctypes binding of liborb_b200.so (include/orb.h): same names, argument
+marshalling only.  Every step of the deposition runs in the library's CUDA
+kernels; there is no CPU fallback, and loading fails loudly if the library has
+not been built (``python -m paper_1908_02219_b200.build``).
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(HERE, "liborb_b200.so")
+
+ORB_OK, ORB_E_INVAL, ORB_E_STATE, ORB_E_NOMEM, ORB_E_CUDA = 0, -1, -2, -3, -4
+ORB_NL_FIXED, ORB_NL_ADAPTIVE = 0, 1
+ORB_DEPOSIT_ZERO_FIRST = 0x1
+ORB_DEPOSIT_NO_BIN = 0x2
+ORB_DEPOSIT_ALGO_ATOMIC = 0x4
+ORB_MARKERS_SORTED = 0x1
+ORB_MAX_NL = 32
+
+# every symbol include/orb.h declares
+SYMBOLS = ("orb_grid_create", "orb_grid_destroy", "orb_grid_shape", "orb_markers_bind",
+           "orb_markers_bin", "orb_deposit", "orb_last_points", "orb_deposit_host",
+           "orb_launch_count", "orb_strerror", "orb_last_error", "orb_version")
+
+
+class OrbError(RuntimeError):
+    def __init__(self, code, msg):
+        super().__init__("liborb_b200: %s (code %d)" % (msg, code))
+        self.code = code
+
+
+class GridDesc(C.Structure):
+    _fields_ = [("ns", C.c_int32), ("ntheta", C.c_int32), ("nphi", C.c_int32),
+                ("r0", C.c_double), ("a", C.c_double), ("b0", C.c_double),
+                ("rho_star", C.c_double), ("q", C.c_double),
+                ("theta_map", C.c_int32), ("device", C.c_int32)]
+
+
+class NlPolicy(C.Structure):
+    _fields_ = [("mode", C.c_int32), ("n_fixed", C.c_int32), ("n_max", C.c_int32),
+                ("flags", C.c_uint32), ("rho_ref", C.c_double), ("alpha0", C.c_double)]
+
+
+_lib = None
+
+
+def lib():
+    """Loads the C-ABI library.  Raises if it is missing: the CUDA path is the only path."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(LIB_PATH):
+        raise OrbError(ORB_E_STATE, "liborb_b200.so is not built at %s; run "
+                       "`python -m paper_1908_02219_b200.build` (nvcc, sm_100a)" % LIB_PATH)
+    L = C.CDLL(LIB_PATH)
+    vp, dp, i64p = C.c_void_p, C.c_void_p, C.POINTER(C.c_int64)
+    L.orb_grid_create.argtypes = [C.POINTER(GridDesc), C.POINTER(vp)]
+    L.orb_grid_destroy.argtypes = [vp]
+    L.orb_grid_shape.argtypes = [vp, C.POINTER(C.c_int64 * 3)]
+    L.orb_markers_bind.argtypes = [vp, C.c_int64, dp, dp, dp, dp, dp, dp, C.c_uint32]
+    L.orb_markers_bin.argtypes = [vp, vp]
+    L.orb_deposit.argtypes = [vp, dp, dp, C.POINTER(NlPolicy), vp]
+    L.orb_last_points.argtypes = [vp, i64p]
+    L.orb_deposit_host.argtypes = [vp, C.c_int64, dp, dp, dp, dp, dp, dp, dp, dp,
+                                   C.POINTER(NlPolicy), i64p, i64p, i64p]
+    L.orb_launch_count.argtypes = [vp, i64p]
+    L.orb_strerror.argtypes = [C.c_int]
+    L.orb_strerror.restype = C.c_char_p
+    L.orb_last_error.argtypes = [vp]
+    L.orb_last_error.restype = C.c_char_p
+    L.orb_version.argtypes = []
+    for name in SYMBOLS:
+        if name not in ("orb_strerror", "orb_last_error"):
+            getattr(L, name).restype = C.c_int
+    _lib = L
+    return L
+
+
+def _check(code, handle=None):
+    if code != ORB_OK:
+        L = lib()
+        msg = L.orb_last_error(handle).decode() if handle else ""
+        raise OrbError(code, msg or L.orb_strerror(code).decode())
+
+
+def _ptr(t):
+    """Address of a torch tensor / numpy array / raw int / None."""
+    if t is None:
+        return None
+    if isinstance(t, int):
+        return t
+    if hasattr(t, "data_ptr"):
+        return t.data_ptr()
+    return t.ctypes.data
+
+
+def policy(n_fixed=4, *, adaptive=False, n_max=None, rho_ref=1.0, alpha0=0.0, flags=0) -> NlPolicy:
+    return NlPolicy(ORB_NL_ADAPTIVE if adaptive else ORB_NL_FIXED, n_fixed,
+                    n_max if n_max is not None else n_fixed, flags, rho_ref, alpha0)
+
+
+class Grid:
+    """RAII wrapper of an orb_grid_t handle; method names follow the C calls."""
+
+    def __init__(self, ns, ntheta, nphi, *, r0=1.0, a=0.3, b0=1.0, rho_star=1.0 / 180.0, q=1.0,
+                 theta_map=1, device=0):
+        self._h = C.c_void_p()
+        self.desc = GridDesc(ns, ntheta, nphi, r0, a, b0, rho_star, q, theta_map, device)
+        _check(lib().orb_grid_create(C.byref(self.desc), C.byref(self._h)))
+        self._keep = None
+
+    def shape(self):
+        dims = (C.c_int64 * 3)()
+        _check(lib().orb_grid_shape(self._h, C.byref(dims)), self._h)
+        return tuple(dims)
+
+    def markers_bind(self, s, theta, phi, vpar, mu, w, flags=0, n=None):
+        if n is None:
+            n = s.numel() if hasattr(s, "numel") else len(s)
+        self._keep = (s, theta, phi, vpar, mu, w)   # the library borrows the pointers
+        _check(lib().orb_markers_bind(self._h, n, _ptr(s), _ptr(theta), _ptr(phi), _ptr(vpar),
+                                      _ptr(mu), _ptr(w), flags), self._h)
+
+    def markers_bin(self, stream=None):
+        _check(lib().orb_markers_bin(self._h, stream), self._h)
+
+    def deposit(self, rho, jpar, pol: NlPolicy, stream=None):
+        _check(lib().orb_deposit(self._h, _ptr(rho), _ptr(jpar), C.byref(pol), stream), self._h)
+
+    def last_points(self) -> int:
+        v = C.c_int64()
+        _check(lib().orb_last_points(self._h, C.byref(v)), self._h)
+        return v.value
+
+    def launch_count(self) -> int:
+        v = C.c_int64()
+        _check(lib().orb_launch_count(self._h, C.byref(v)), self._h)
+        return v.value
+
+    def deposit_host(self, s, theta, phi, vpar, mu, w, rho_host, jpar_host, pol: NlPolicy, n=None):
+        """Host arrays in, host grids out (overwritten). -> (n_points, h2d_bytes, d2h_bytes)."""
+        if n is None:
+            n = s.numel() if hasattr(s, "numel") else len(s)
+        npts, up, down = C.c_int64(), C.c_int64(), C.c_int64()
+        _check(lib().orb_deposit_host(self._h, n, _ptr(s), _ptr(theta), _ptr(phi), _ptr(vpar),
+                                      _ptr(mu), _ptr(w), _ptr(rho_host), _ptr(jpar_host),
+                                      C.byref(pol), C.byref(npts), C.byref(up), C.byref(down)),
+               self._h)
+        return npts.value, up.value, down.value
+
+    def destroy(self):
+        if self._h:
+            lib().orb_grid_destroy(self._h)
+            self._h = C.c_void_p()
+            self._keep = None
+
+    def __del__(self):
+        try:
+            self.destroy()
+        except Exception:
+            pass
+
+    def __enter__(self):
+        return self
+
+    def __exit__(self, *exc):
+        self.destroy()
+
+
+def grid_for(cfg, device=0) -> Grid:
+    """Grid handle for a workloads.Config."""
+    return Grid(cfg.ns, cfg.ntheta, cfg.nphi, r0=cfg.r0, a=cfg.a, b0=cfg.b0, rho_star=cfg.rho_star,
+                q=cfg.q, device=device)
+
+
+def policy_for(cfg, flags=0) -> NlPolicy:
+    return policy(cfg.n_fixed, adaptive=cfg.adaptive, n_max=cfg.n_max if cfg.adaptive else None,
+                  rho_ref=cfg.rho_ref, flags=flags)

@@ -1,0 +1,411 @@
+// C ABI of liborb_b200 (include/orb.h): handle, scratch ownership, argument
+// checks, launches.  No arithmetic of the method lives here.
+#include <math.h>
+#include <stdio.h>
+#include <string.h>
+
+#include <new>
+#include <vector>
+
+#include "orb_internal.h"
+
+using namespace orb;
+
+struct orb_grid {
+  orb_grid_desc_t desc;
+  int64_t ncells;
+  int64_t nnodes;
+
+  // bound markers (borrowed) and binning state
+  Markers bound;
+  uint32_t bind_flags;
+  bool have_bind;
+  bool binned;
+
+  // scratch (owned)
+  BinScratch bin;
+  int64_t bin_capacity;      // markers the rank/rec buffers can hold
+  double2* ring;             // device ring table
+  double ring_alpha0;
+  bool ring_valid;
+  unsigned long long* d_points;
+
+  // orb_deposit_host staging (owned)
+  double* hbuf[6];
+  int64_t hbuf_capacity;
+  double* hgrid[2];
+
+  int64_t launches;
+  char err[512];
+};
+
+namespace {
+
+struct DeviceGuard {
+  int prev;
+  bool ok;
+  explicit DeviceGuard(int dev) : prev(-1), ok(false) {
+    if (cudaGetDevice(&prev) != cudaSuccess) { prev = -1; }
+    ok = (cudaSetDevice(dev) == cudaSuccess);
+  }
+  ~DeviceGuard() {
+    if (prev >= 0) cudaSetDevice(prev);
+  }
+};
+
+int fail(orb_grid* g, int code, const char* what, cudaError_t ce = cudaSuccess) {
+  if (g) {
+    if (ce != cudaSuccess)
+      snprintf(g->err, sizeof(g->err), "%s: %s (%s)", orb_strerror(code), what,
+               cudaGetErrorString(ce));
+    else
+      snprintf(g->err, sizeof(g->err), "%s: %s", orb_strerror(code), what);
+  }
+  return code;
+}
+
+#define ORB_CUDA(g, call)                                           \
+  do {                                                              \
+    cudaError_t ce__ = (call);                                      \
+    if (ce__ != cudaSuccess) {                                      \
+      cudaGetLastError();                                           \
+      return fail((g), ce__ == cudaErrorMemoryAllocation ? ORB_E_NOMEM : ORB_E_CUDA, #call, ce__); \
+    }                                                               \
+  } while (0)
+
+bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
+
+Params make_params(const orb_grid* g, const orb_nl_policy_t* pol) {
+  Params P;
+  P.ns = g->desc.ns;
+  P.nth = g->desc.ntheta;
+  P.nph = g->desc.nphi;
+  P.theta_map = g->desc.theta_map;
+  P.eps = g->desc.a / g->desc.r0;
+  P.b0 = g->desc.b0;
+  P.rho_star = g->desc.rho_star;
+  P.q = g->desc.q;
+  P.nth_scale = (double)g->desc.ntheta / kTwoPi;
+  P.nph_scale = (double)g->desc.nphi / kTwoPi;
+  P.adaptive = 0;
+  P.n_fixed = 1;
+  P.n_max = 1;
+  P.rho_ref = 1.0;
+  if (pol) {
+    P.adaptive = pol->mode == ORB_NL_ADAPTIVE;
+    P.n_fixed = pol->n_fixed;
+    P.n_max = P.adaptive ? pol->n_max : pol->n_fixed;
+    P.rho_ref = P.adaptive ? pol->rho_ref : 1.0;
+  }
+  P.ring = g->ring;
+  return P;
+}
+
+int check_policy(orb_grid* g, const orb_nl_policy_t* pol) {
+  if (!pol) return fail(g, ORB_E_INVAL, "policy is NULL");
+  if (pol->mode != ORB_NL_FIXED && pol->mode != ORB_NL_ADAPTIVE)
+    return fail(g, ORB_E_INVAL, "policy.mode");
+  if (pol->n_fixed < 1 || pol->n_fixed > ORB_MAX_NL)
+    return fail(g, ORB_E_INVAL, "policy.n_fixed out of [1, ORB_MAX_NL]");
+  if (pol->mode == ORB_NL_ADAPTIVE) {
+    if (pol->n_max < pol->n_fixed || pol->n_max > ORB_MAX_NL)
+      return fail(g, ORB_E_INVAL, "policy.n_max out of [n_fixed, ORB_MAX_NL]");
+    if (!(pol->rho_ref > 0.0) || !isfinite(pol->rho_ref))
+      return fail(g, ORB_E_INVAL, "policy.rho_ref must be > 0");
+  }
+  if (!isfinite(pol->alpha0)) return fail(g, ORB_E_INVAL, "policy.alpha0");
+  return ORB_OK;
+}
+
+// (cos, sin)(alpha0 + 2 pi l / N) for N = 1..ORB_MAX_NL, l < N; entry at N(N-1)/2 + l.
+int upload_ring(orb_grid* g, double alpha0, cudaStream_t st) {
+  if (g->ring_valid && g->ring_alpha0 == alpha0) return ORB_OK;
+  const int total = ORB_MAX_NL * (ORB_MAX_NL + 1) / 2;
+  std::vector<double2> h(total);
+  for (int n = 1; n <= ORB_MAX_NL; ++n)
+    for (int l = 0; l < n; ++l) {
+      const double al = alpha0 + kTwoPi * (double)l / (double)n;
+      h[n * (n - 1) / 2 + l] = make_double2(cos(al), sin(al));
+    }
+  // pageable source: the copy is staged before the call returns
+  ORB_CUDA(g, cudaMemcpyAsync(g->ring, h.data(), total * sizeof(double2), cudaMemcpyHostToDevice, st));
+  ORB_CUDA(g, cudaStreamSynchronize(st));
+  g->ring_alpha0 = alpha0;
+  g->ring_valid = true;
+  return ORB_OK;
+}
+
+void free_bin(orb_grid* g) {
+  cudaFree(g->bin.rank);
+  cudaFree(g->bin.rec);
+  g->bin.rank = nullptr;
+  g->bin.rec = nullptr;
+  g->bin_capacity = 0;
+}
+
+int ensure_bin_scratch(orb_grid* g, int64_t n, bool need_records) {
+  if (!g->bin.cell_start) {
+    ORB_CUDA(g, cudaMalloc(&g->bin.cell_start, (size_t)(g->ncells + 1) * sizeof(uint32_t)));
+    const int64_t nb = (g->ncells + 4095) / 4096 + 1;
+    ORB_CUDA(g, cudaMalloc(&g->bin.block_sums, (size_t)nb * sizeof(uint32_t)));
+  }
+  if (need_records && n > g->bin_capacity) {
+    free_bin(g);
+    ORB_CUDA(g, cudaMalloc(&g->bin.rank, (size_t)n * sizeof(uint32_t)));
+    ORB_CUDA(g, cudaMalloc(&g->bin.rec, (size_t)n * kRecDoubles * sizeof(double)));
+    g->bin_capacity = n;
+  }
+  return ORB_OK;
+}
+
+int do_bin(orb_grid* g, cudaStream_t st) {
+  const bool presorted = (g->bind_flags & ORB_MARKERS_SORTED) != 0;
+  int rc = ensure_bin_scratch(g, g->bound.n, !presorted);
+  if (rc != ORB_OK) return rc;
+  Params P = make_params(g, nullptr);
+  Markers M = g->bound;
+  M.rec = nullptr;
+  int l = launch_bin(P, M, g->bin, presorted, st);
+  if (l < 0) return fail(g, ORB_E_CUDA, "binning launch", cudaGetLastError());
+  g->launches += l;
+  ORB_CUDA(g, cudaGetLastError());
+  g->binned = true;
+  return ORB_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+int orb_version(void) { return ORB_VERSION; }
+
+const char* orb_strerror(int code) {
+  switch (code) {
+    case ORB_OK: return "ok";
+    case ORB_E_INVAL: return "invalid argument";
+    case ORB_E_STATE: return "invalid call order";
+    case ORB_E_NOMEM: return "out of device memory";
+    case ORB_E_CUDA: return "CUDA error";
+    default: return "unknown status";
+  }
+}
+
+const char* orb_last_error(const orb_grid_t* g) { return g ? g->err : ""; }
+
+int orb_grid_create(const orb_grid_desc_t* d, orb_grid_t** out) {
+  if (!d || !out) return ORB_E_INVAL;
+  if (d->ns < 4 || d->ntheta < 4 || d->nphi < 4) return ORB_E_INVAL;
+  if (!(d->r0 > 0.0) || !(d->a > 0.0) || !(d->a < d->r0) || !(d->b0 > 0.0)) return ORB_E_INVAL;
+  if (!(d->rho_star >= 0.0) || !isfinite(d->rho_star) || !isfinite(d->q)) return ORB_E_INVAL;
+  if (d->theta_map != 0 && d->theta_map != 1) return ORB_E_INVAL;
+  const int64_t ncells = (int64_t)d->ns * d->ntheta * d->nphi;
+  const int64_t nnodes = (int64_t)(d->ns + 3) * d->ntheta * d->nphi;
+  if (ncells >= (int64_t)1 << 31) return ORB_E_INVAL;
+  int ndev = 0;
+  if (cudaGetDeviceCount(&ndev) != cudaSuccess || d->device < 0 || d->device >= ndev) {
+    cudaGetLastError();
+    return ORB_E_CUDA;
+  }
+  DeviceGuard dg(d->device);
+  if (!dg.ok) return ORB_E_CUDA;
+  orb_grid* g = new (std::nothrow) orb_grid();
+  if (!g) return ORB_E_NOMEM;
+  memset(g, 0, sizeof(*g));
+  g->desc = *d;
+  g->ncells = ncells;
+  g->nnodes = nnodes;
+  g->bin.ncells = ncells;
+  const int total = ORB_MAX_NL * (ORB_MAX_NL + 1) / 2;
+  if (cudaMalloc(&g->ring, total * sizeof(double2)) != cudaSuccess ||
+      cudaMalloc(&g->d_points, sizeof(unsigned long long)) != cudaSuccess ||
+      cudaMemset(g->d_points, 0, sizeof(unsigned long long)) != cudaSuccess) {
+    cudaGetLastError();
+    cudaFree(g->ring);
+    cudaFree(g->d_points);
+    delete g;
+    return ORB_E_CUDA;
+  }
+  *out = g;
+  return ORB_OK;
+}
+
+int orb_grid_destroy(orb_grid_t* g) {
+  if (!g) return ORB_OK;
+  DeviceGuard dg(g->desc.device);
+  cudaDeviceSynchronize();
+  free_bin(g);
+  cudaFree(g->bin.cell_start);
+  cudaFree(g->bin.block_sums);
+  cudaFree(g->ring);
+  cudaFree(g->d_points);
+  for (int i = 0; i < 6; ++i) cudaFree(g->hbuf[i]);
+  cudaFree(g->hgrid[0]);
+  cudaFree(g->hgrid[1]);
+  cudaGetLastError();
+  delete g;
+  return ORB_OK;
+}
+
+int orb_grid_shape(const orb_grid_t* g, int64_t dims[3]) {
+  if (!g || !dims) return ORB_E_INVAL;
+  dims[0] = g->desc.ns + 3;
+  dims[1] = g->desc.ntheta;
+  dims[2] = g->desc.nphi;
+  return ORB_OK;
+}
+
+int orb_markers_bind(orb_grid_t* g, int64_t n, const double* s, const double* theta,
+                     const double* phi, const double* vpar, const double* mu, const double* w,
+                     uint32_t flags) {
+  if (!g) return ORB_E_INVAL;
+  if (n < 0) return fail(g, ORB_E_INVAL, "n < 0");
+  if (n >= ((int64_t)1 << 32) - 1) return fail(g, ORB_E_INVAL, "n too large");
+  if (flags & ~ORB_MARKERS_SORTED) return fail(g, ORB_E_INVAL, "unknown bind flag");
+  if (n > 0 && (!s || !theta || !phi || !mu || !w)) return fail(g, ORB_E_INVAL, "NULL marker array");
+  if (!aligned16(s) || !aligned16(theta) || !aligned16(phi) || !aligned16(vpar) ||
+      !aligned16(mu) || !aligned16(w))
+    return fail(g, ORB_E_INVAL, "marker arrays must be 16-byte aligned");
+  g->bound.s = s;
+  g->bound.th = theta;
+  g->bound.ph = phi;
+  g->bound.vpar = vpar;
+  g->bound.mu = mu;
+  g->bound.w = w;
+  g->bound.rec = nullptr;
+  g->bound.n = n;
+  g->bind_flags = flags;
+  g->have_bind = true;
+  g->binned = false;
+  g->err[0] = 0;
+  return ORB_OK;
+}
+
+int orb_markers_bin(orb_grid_t* g, void* stream) {
+  if (!g) return ORB_E_INVAL;
+  if (!g->have_bind) return fail(g, ORB_E_STATE, "orb_markers_bin before orb_markers_bind");
+  DeviceGuard dg(g->desc.device);
+  if (!dg.ok) return fail(g, ORB_E_CUDA, "cudaSetDevice");
+  return do_bin(g, static_cast<cudaStream_t>(stream));
+}
+
+int orb_deposit(orb_grid_t* g, double* rho, double* jpar, const orb_nl_policy_t* pol,
+                void* stream) {
+  if (!g) return ORB_E_INVAL;
+  if (!rho) return fail(g, ORB_E_INVAL, "rho is NULL");
+  if (!aligned16(rho) || !aligned16(jpar)) return fail(g, ORB_E_INVAL, "grids must be 16-byte aligned");
+  int rc = check_policy(g, pol);
+  if (rc != ORB_OK) return rc;
+  if (!g->have_bind) return fail(g, ORB_E_STATE, "orb_deposit before orb_markers_bind");
+  if (jpar && !g->bound.vpar && g->bound.n > 0)
+    return fail(g, ORB_E_INVAL, "jpar requested but markers were bound without vpar");
+  DeviceGuard dg(g->desc.device);
+  if (!dg.ok) return fail(g, ORB_E_CUDA, "cudaSetDevice");
+  cudaStream_t st = static_cast<cudaStream_t>(stream);
+
+  rc = upload_ring(g, pol->alpha0, st);
+  if (rc != ORB_OK) return rc;
+  const bool atomic_algo = (pol->flags & ORB_DEPOSIT_ALGO_ATOMIC) != 0;
+  const bool no_bin = (pol->flags & ORB_DEPOSIT_NO_BIN) != 0;
+  if (!no_bin && !atomic_algo && !g->binned) {
+    rc = do_bin(g, st);
+    if (rc != ORB_OK) return rc;
+  }
+  if (pol->flags & ORB_DEPOSIT_ZERO_FIRST) {
+    ORB_CUDA(g, cudaMemsetAsync(rho, 0, (size_t)g->nnodes * sizeof(double), st));
+    if (jpar) ORB_CUDA(g, cudaMemsetAsync(jpar, 0, (size_t)g->nnodes * sizeof(double), st));
+  }
+  ORB_CUDA(g, cudaMemsetAsync(g->d_points, 0, sizeof(unsigned long long), st));
+
+  Params P = make_params(g, pol);
+  Markers M = g->bound;
+  const bool use_binned = g->binned && !no_bin;
+  const bool presorted = (g->bind_flags & ORB_MARKERS_SORTED) != 0;
+  if (use_binned && !presorted) M.rec = g->bin.rec;
+  int l;
+  if (atomic_algo || !use_binned) {
+    l = launch_deposit_atomic(P, M, rho, jpar, g->d_points, st);
+  } else {
+    l = launch_deposit_tile(P, M, g->bin.cell_start, rho, jpar, g->d_points, st);
+  }
+  if (l < 0) return fail(g, ORB_E_CUDA, "deposit launch", cudaGetLastError());
+  g->launches += l;
+  ORB_CUDA(g, cudaGetLastError());
+  return ORB_OK;
+}
+
+int orb_last_points(orb_grid_t* g, int64_t* n_points) {
+  if (!g || !n_points) return ORB_E_INVAL;
+  DeviceGuard dg(g->desc.device);
+  unsigned long long v = 0;
+  // default-stream copy: waits for prior work on blocking streams; then make sure
+  ORB_CUDA(g, cudaDeviceSynchronize());
+  ORB_CUDA(g, cudaMemcpy(&v, g->d_points, sizeof(v), cudaMemcpyDeviceToHost));
+  *n_points = (int64_t)v;
+  return ORB_OK;
+}
+
+int orb_launch_count(const orb_grid_t* g, int64_t* n) {
+  if (!g || !n) return ORB_E_INVAL;
+  *n = g->launches;
+  return ORB_OK;
+}
+
+int orb_deposit_host(orb_grid_t* g, int64_t n, const double* s, const double* theta,
+                     const double* phi, const double* vpar, const double* mu, const double* w,
+                     double* rho_host, double* jpar_host, const orb_nl_policy_t* pol,
+                     int64_t* n_points, int64_t* h2d_bytes, int64_t* d2h_bytes) {
+  if (!g) return ORB_E_INVAL;
+  if (n < 0 || !rho_host) return fail(g, ORB_E_INVAL, "n < 0 or rho_host NULL");
+  if (n > 0 && (!s || !theta || !phi || !mu || !w)) return fail(g, ORB_E_INVAL, "NULL marker array");
+  if (jpar_host && !vpar && n > 0) return fail(g, ORB_E_INVAL, "jpar_host needs vpar");
+  int rc = check_policy(g, pol);
+  if (rc != ORB_OK) return rc;
+  DeviceGuard dg(g->desc.device);
+  if (!dg.ok) return fail(g, ORB_E_CUDA, "cudaSetDevice");
+  if (n > g->hbuf_capacity) {
+    for (int i = 0; i < 6; ++i) {
+      cudaFree(g->hbuf[i]);
+      g->hbuf[i] = nullptr;
+    }
+    g->hbuf_capacity = 0;
+    for (int i = 0; i < 6; ++i) ORB_CUDA(g, cudaMalloc(&g->hbuf[i], (size_t)n * sizeof(double)));
+    g->hbuf_capacity = n;
+  }
+  for (int i = 0; i < 2; ++i)
+    if (!g->hgrid[i]) ORB_CUDA(g, cudaMalloc(&g->hgrid[i], (size_t)g->nnodes * sizeof(double)));
+  const double* src[6] = {s, theta, phi, vpar, mu, w};
+  int64_t up = 0, down = 0;
+  cudaStream_t st = 0;
+  for (int i = 0; i < 6; ++i) {
+    if (!src[i] || n == 0) continue;
+    ORB_CUDA(g, cudaMemcpyAsync(g->hbuf[i], src[i], (size_t)n * sizeof(double),
+                                cudaMemcpyHostToDevice, st));
+    up += n * (int64_t)sizeof(double);
+  }
+  rc = orb_markers_bind(g, n, g->hbuf[0], g->hbuf[1], g->hbuf[2], vpar ? g->hbuf[3] : nullptr,
+                        g->hbuf[4], g->hbuf[5], 0);
+  if (rc != ORB_OK) return rc;
+  orb_nl_policy_t p2 = *pol;
+  p2.flags |= ORB_DEPOSIT_ZERO_FIRST;
+  rc = orb_deposit(g, g->hgrid[0], jpar_host ? g->hgrid[1] : nullptr, &p2, st);
+  if (rc != ORB_OK) return rc;
+  ORB_CUDA(g, cudaMemcpyAsync(rho_host, g->hgrid[0], (size_t)g->nnodes * sizeof(double),
+                              cudaMemcpyDeviceToHost, st));
+  down += g->nnodes * (int64_t)sizeof(double);
+  if (jpar_host) {
+    ORB_CUDA(g, cudaMemcpyAsync(jpar_host, g->hgrid[1], (size_t)g->nnodes * sizeof(double),
+                                cudaMemcpyDeviceToHost, st));
+    down += g->nnodes * (int64_t)sizeof(double);
+  }
+  ORB_CUDA(g, cudaStreamSynchronize(st));
+  if (n_points) {
+    unsigned long long v = 0;
+    ORB_CUDA(g, cudaMemcpy(&v, g->d_points, sizeof(v), cudaMemcpyDeviceToHost));
+    *n_points = (int64_t)v;
+  }
+  if (h2d_bytes) *h2d_bytes = up;
+  if (d2h_bytes) *d2h_bytes = down;
+  return ORB_OK;
+}
+
+}  // extern "C"

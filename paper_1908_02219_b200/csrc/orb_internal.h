@@ -1,0 +1,64 @@
+// Internal declarations shared by the translation units of liborb_b200.
+// Not part of the public ABI (see include/orb.h).
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "orb.h"
+
+namespace orb {
+
+constexpr double kTwoPi = 6.283185307179586476925286766559;
+constexpr int kRecDoubles = 6;  // binned marker record: s, theta*, phi, vpar, mu, w
+
+// Everything a kernel needs to know about grid, geometry, species and N_L policy.
+// Passed by value as a kernel parameter.
+struct Params {
+  int ns, nth, nph;      // cells
+  int theta_map;
+  double eps;            // a / r0
+  double b0;
+  double rho_star;
+  double q;
+  double nth_scale;      // ntheta / 2pi
+  double nph_scale;      // nphi / 2pi
+  // N_L policy
+  int adaptive;
+  int n_fixed;           // N_L, or n_min when adaptive
+  int n_max;
+  double rho_ref;
+  // ring table: entry (N, l) at N*(N-1)/2 + l holds (cos, sin)(alpha0 + 2 pi l / N), N = 1..ORB_MAX_NL
+  const double2* ring;
+};
+
+// Bound markers: either the caller's SoA arrays (in bound order) or the library's
+// binned array-of-records scratch (rec != nullptr), 6 doubles per marker.
+struct Markers {
+  const double* s;
+  const double* th;
+  const double* ph;
+  const double* vpar;   // may be nullptr
+  const double* mu;
+  const double* w;
+  const double* rec;    // binned records, or nullptr
+  int64_t n;
+};
+
+// ---- kernels' host-side launchers (each returns the number of kernels it launched, <0 on error)
+int launch_deposit_atomic(const Params& P, const Markers& M, double* rho, double* jpar,
+                          unsigned long long* d_points, cudaStream_t st);
+
+struct BinScratch {
+  uint32_t* rank;        // n
+  uint32_t* cell_start;  // ncells + 1 (counts during pass 1, exclusive offsets afterwards)
+  uint32_t* block_sums;  // scan scratch
+  double* rec;           // n * kRecDoubles
+  int64_t ncells;
+};
+int launch_bin(const Params& P, const Markers& M, const BinScratch& B, bool presorted,
+               cudaStream_t st);
+
+int launch_deposit_tile(const Params& P, const Markers& M, const uint32_t* cell_start, double* rho,
+                        double* jpar, unsigned long long* d_points, cudaStream_t st);
+
+}  // namespace orb
