@@ -1,0 +1,370 @@
+#!/usr/bin/env python
+"""bench.py -- the measurement contract.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload cfg3] [--impl ours|reference]
+
+One STEP = one pass of the whole hot path over one batch of
+synthetic markers in random order: bind -> bin (counting sort by cell) -> zero grids -> tile
+deposit of charge (+ parallel current).  Default workload: BASELINE.json configs[3] (the config
+the >= 50 % HBM-roofline target is quoted on; 2^26 markers, 256x512x128 cells, N_L = 4, rho and
+j_par), which fits one B200.
+
+Prints ONE JSON line (rank 0).  `value` = Larmor points/s of the whole job with the markers
+already resident in HBM; `e2e` = the same through orb_deposit_host with HOST (pinned) marker
+arrays and host grids, copies inside the timed region; `roofline` = algorithmic bytes of the
+deposit kernel / its CUDA-event duration against MEASURED_PEAKS.json; `cpu_baseline` = the
+CPU oracle, as it stands, on a bounded sample of the same workload.
+
+`--impl reference` times the oracle (single thread, host cores) on the same workload, each
+step a bounded sample; rank 0 only.
+"""
+from __future__ import annotations
+
+import argparse
+import dataclasses
+import json
+import os
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import numpy as np  # noqa: E402
+
+from paper_1908_02219_b200 import replicas as R  # noqa: E402
+from paper_1908_02219_b200 import workloads as W  # noqa: E402
+
+METRIC = "gyro-averaged Larmor points deposited/sec and achieved HBM GB/s (% of roofline)"
+UNIT = "Larmor points/s"
+HBM_FALLBACK_GBS = 6650.0      # /opt/skills/guides/B200_PROFILING.md fallback
+HBM_NOMINAL_GBS = 8000.0       # the "~8 TB/s" north_star quotes
+L2_BYTES = 126 << 20
+
+# dram__bytes_read.sum + dram__bytes_write.sum of ONE launch of the deposit kernel, from the
+# `ncu --set full` capture summarised in profiles/ (None until a capture of that workload exists)
+NCU_TRAFFIC_BYTES = {}
+
+
+def measured_hbm_peak():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    try:
+        with open(p) as f:
+            return float(json.load(f)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    except Exception:
+        return HBM_FALLBACK_GBS, "fallback (B200_PROFILING.md)"
+
+
+class ClockSampler:
+    """Samples SM clock and throttle reasons through NVML while the timed region runs."""
+
+    REASONS = {
+        0x1: "gpu_idle", 0x2: "applications_clocks_setting", 0x4: "sw_power_cap",
+        0x8: "hw_slowdown", 0x10: "sync_boost", 0x20: "sw_thermal_slowdown",
+        0x40: "hw_thermal_slowdown", 0x80: "hw_power_brake_slowdown", 0x100: "display_clock_setting",
+    }
+
+    def __init__(self, index=0, period_s=0.004):
+        self.index, self.period = index, period_s
+        self.samples, self.reasons, self.sm_max = [], set(), None
+        self._stop = threading.Event()
+        self._thr = None
+        self.ok = False
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            self.nv = pynvml
+            self.h = pynvml.nvmlDeviceGetHandleByIndex(index)
+            self.sm_max = int(pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM))
+            self.ok = True
+        except Exception as e:  # noqa: BLE001
+            self.err = repr(e)
+
+    def _loop(self):
+        nv = self.nv
+        while not self._stop.is_set():
+            try:
+                self.samples.append(int(nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM)))
+                bits = int(nv.nvmlDeviceGetCurrentClocksEventReasons(self.h))
+                for b, name in self.REASONS.items():
+                    if bits & b and name != "gpu_idle":
+                        self.reasons.add(name)
+            except Exception:  # noqa: BLE001
+                pass
+            self._stop.wait(self.period)
+
+    def start(self):
+        if self.ok:
+            self._thr = threading.Thread(target=self._loop, daemon=True)
+            self._thr.start()
+
+    def stop(self):
+        if self._thr:
+            self._stop.set()
+            self._thr.join()
+
+    def summary(self):
+        if not self.ok or not self.samples:
+            return {"sm_mhz": None, "sm_max_mhz": self.sm_max, "reasons": [], "samples": 0}
+        return {"sm_mhz": float(np.median(self.samples)), "sm_max_mhz": self.sm_max,
+                "reasons": sorted(self.reasons), "samples": len(self.samples)}
+
+
+def pick_config(name: str, rank: int):
+    cfg = W.CONFIGS[name]
+    return dataclasses.replace(cfg, seed=R.replica_seed(cfg.seed, rank))
+
+
+def config_json(cfg, world, extra=None):
+    c = {"workload": "%s: grid %dx%dx%d cells, %d markers fp64 SoA, %s N_L%s, rho_star=1/%d, %s, %s order"
+         % (cfg.name, cfg.ns, cfg.ntheta, cfg.nphi, cfg.n_markers,
+            "adaptive" if cfg.adaptive else "fixed",
+            ("=4..%d" % cfg.n_max) if cfg.adaptive else ("=%d" % cfg.n_fixed),
+            round(1 / cfg.rho_star), "rho+jpar" if cfg.current else "rho only", cfg.order),
+         "step": "bind + bin (counting sort by cell) + zero grids + tile deposit",
+         "l2_policy": "inputs (%.2f GB markers) larger than the 126 MB L2; no flush needed"
+                      % (cfg.n_markers * 48 / 1e9),
+         "parallelism": "replicas x%d (no sharding, no collective)" % world if world > 1 else "1 GPU"}
+    if extra:
+        c.update(extra)
+    return c
+
+
+def oracle_sample(cfg, m, n_sample):
+    """Times the oracle, single-threaded and as it stands, on the first n_sample markers."""
+    import oracle as O
+    og = O.geom(cfg.ns, cfg.ntheta, cfg.nphi, r0=cfg.r0, a=cfg.a, b0=cfg.b0, rho_star=cfg.rho_star,
+                q=cfg.q)
+    op = (O.policy_adaptive(cfg.n_fixed, cfg.n_max, cfg.rho_ref) if cfg.adaptive
+          else O.policy_fixed(cfg.n_fixed))
+    O.lib()
+    arrs = [np.ascontiguousarray(m[f][:n_sample]) for f in W.FIELDS]
+    shape = O.grid_shape(og)
+    rho = np.zeros(shape)
+    jpar = np.zeros(shape) if cfg.current else None
+    t0 = time.perf_counter()
+    _, _, npts = O.deposit(og, op, *arrs, current=cfg.current, rho=rho, jpar=jpar)
+    dt = time.perf_counter() - t0
+    return npts, dt
+
+
+# ------------------------------------------------------------------------------------------
+def run_reference(args):
+    rank, _, world = R.env_rank()
+    if rank != 0:
+        return 0
+    cfg = pick_config(args.workload, 0)
+    n_sample = min(args.ref_sample, cfg.n_markers)
+    m = W.generate(W.scaled(cfg, n_sample))
+    for _ in range(args.warmup):
+        oracle_sample(cfg, m, n_sample)
+    pts, secs = 0, 0.0
+    for _ in range(args.steps):
+        n, dt = oracle_sample(cfg, m, n_sample)
+        pts += n
+        secs += dt
+    value = pts / secs
+    sample = "first %d markers of %s per step (%d Larmor points), single thread" % (
+        n_sample, cfg.name, pts // max(args.steps, 1))
+    line = {
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * secs / args.steps,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+        "data": "synthetic", "config": config_json(cfg, 1, {"step": "oracle_deposit on a bounded sample"}),
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0, "host_cores": os.cpu_count(),
+    }
+    print(json.dumps(line), flush=True)
+    return 0
+
+
+# ------------------------------------------------------------------------------------------
+def run_ours(args):
+    import torch
+
+    from paper_1908_02219_b200 import binding as B
+    from paper_1908_02219_b200 import build as build_mod
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the CUDA path is the only path (no CPU fallback)")
+    rank, local_rank, world = R.init()
+    if world != args.gpus and world > 1:
+        raise SystemExit("bench.py: --gpus %d but WORLD_SIZE=%d" % (args.gpus, world))
+    torch.cuda.set_device(local_rank)
+    dev = torch.device("cuda", local_rank)
+    if rank == 0:
+        build_mod.build()
+    R.barrier()
+    B.lib()
+
+    cfg = pick_config(args.workload, rank)
+    n = cfg.n_markers
+    # inputs: generated on the host into pinned memory (they are the e2e leg's source)
+    host = {f: torch.empty(n, dtype=torch.float64, pin_memory=True) for f in W.FIELDS}
+    m = {f: host[f].numpy() for f in W.FIELDS}
+    W.generate(cfg, out=m)
+    d = {f: host[f].to(dev, non_blocking=True) for f in W.FIELDS}
+    torch.cuda.synchronize()
+
+    g = B.grid_for(cfg, device=local_rank)
+    shape = g.shape()
+    rho = torch.zeros(shape, dtype=torch.float64, device=dev)
+    jpar = torch.zeros(shape, dtype=torch.float64, device=dev) if cfg.current else None
+    pol = B.policy_for(cfg)
+    bind_flags = B.ORB_MARKERS_SORTED if cfg.order == "sorted" else 0
+    stream = torch.cuda.current_stream()
+    st = stream.cuda_stream
+
+    def step(evs=None):
+        g.markers_bind(d["s"], d["theta"], d["phi"], d["vpar"] if cfg.current else None, d["mu"],
+                       d["w"], flags=bind_flags)
+        if evs:
+            evs[0].record(stream)
+        g.markers_bin(st)
+        if evs:
+            evs[1].record(stream)
+        g.grid_zero(rho, jpar, st)
+        if evs:
+            evs[2].record(stream)
+        g.deposit(rho, jpar, pol, st)
+        if evs:
+            evs[3].record(stream)
+
+    for _ in range(args.warmup):
+        step()
+    torch.cuda.synchronize()
+    npts_step = g.last_points()
+
+    K = args.steps
+    evs = [[torch.cuda.Event(enable_timing=True) for _ in range(4)] for _ in range(K)]
+    e_start, e_end = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    sampler = ClockSampler(index=local_rank)
+    launches0 = g.launch_count()
+    R.barrier()
+    torch.cuda.synchronize()
+    sampler.start()
+    e_start.record(stream)
+    for k in range(K):
+        step(evs[k])
+    e_end.record(stream)
+    torch.cuda.synchronize()
+    R.barrier()
+    sampler.stop()
+    launches = g.launch_count() - launches0
+    total_ms = e_start.elapsed_time(e_end)
+    bin_ms = sum(e[0].elapsed_time(e[1]) for e in evs) / K
+    zero_ms = sum(e[1].elapsed_time(e[2]) for e in evs) / K
+    dep_ms_all = [e[2].elapsed_time(e[3]) for e in evs]
+    dep_ms = sum(dep_ms_all) / K
+    assert g.last_points() == npts_step
+
+    # result sanity inside the bench: charge conservation (P1) of the last step
+    q_sum = float(rho.sum().item())
+    w_sum = float(d["w"].sum().item()) * cfg.q
+    w_abs = float(d["w"].abs().sum().item()) * abs(cfg.q)
+    conservation = abs(q_sum - w_sum) / w_abs
+
+    job_ms, job_pts = R.combine(total_ms, float(npts_step) * K, device=dev)
+    value = job_pts / (job_ms * 1e-3)
+
+    # ---- e2e: HOST marker arrays -> orb_deposit_host -> HOST grids, every step
+    E = max(1, min(args.e2e_steps, K))
+    rho_h = torch.empty(shape, dtype=torch.float64, pin_memory=True)
+    jpar_h = torch.empty(shape, dtype=torch.float64, pin_memory=True) if cfg.current else None
+    del d
+    torch.cuda.empty_cache()
+
+    def e2e_step():
+        return g.deposit_host(m["s"], m["theta"], m["phi"], m["vpar"] if cfg.current else None,
+                              m["mu"], m["w"], rho_h.numpy(), jpar_h.numpy() if cfg.current else None,
+                              pol)
+
+    e2e_step()
+    torch.cuda.synchronize()
+    launches_e0 = g.launch_count()
+    R.barrier()
+    torch.cuda.synchronize()
+    t0 = time.perf_counter()
+    for _ in range(E):
+        npts_e, up, down = e2e_step()
+    torch.cuda.synchronize()
+    e2e_ms = (time.perf_counter() - t0) * 1e3
+    R.barrier()
+    launches_e = g.launch_count() - launches_e0
+    e2e_job_ms, e2e_job_pts = R.combine(e2e_ms, float(npts_e) * E, device=dev)
+    e2e_value = e2e_job_pts / (e2e_job_ms * 1e-3)
+    e2e_conservation = abs(float(rho_h.sum().item()) - w_sum) / w_abs
+    g.destroy()
+
+    line = None
+    if rank == 0:
+        peak, peak_src = measured_hbm_peak()
+        alg_bytes = cfg.algorithmic_bytes
+        achieved = alg_bytes / (dep_ms * 1e-3) / 1e9
+        line = {
+            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K,
+            "warmup": args.warmup, "ms_per_step": job_ms / K, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": config_json(cfg, world),
+            "points_per_step": npts_step,
+            "phases_ms": {"bin": bin_ms, "zero": zero_ms, "deposit": dep_ms,
+                          "deposit_min": min(dep_ms_all), "deposit_max": max(dep_ms_all)},
+            "deposit_only": {"value": npts_step / (dep_ms * 1e-3), "unit": UNIT,
+                             "note": "tile deposit kernel on already-binned markers"},
+            "step_hbm": {"achieved": alg_bytes * K / (total_ms * 1e-3) / 1e9, "unit": "GB/s",
+                         "frac": alg_bytes * K / (total_ms * 1e-3) / 1e9 / peak,
+                         "note": "same algorithmic bytes over the whole step (bin + zero + deposit)"},
+            "roofline": {"bound": "hbm", "kernel": "k_deposit_tile", "achieved": achieved,
+                         "peak": peak, "unit": "GB/s", "frac": achieved / peak,
+                         "traffic": NCU_TRAFFIC_BYTES.get(cfg.name), "peak_source": peak_src,
+                         "algorithmic_bytes": alg_bytes, "kernel_ms": dep_ms,
+                         "frac_of_nominal_8TBs": achieved / HBM_NOMINAL_GBS},
+            "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": up,
+                    "d2h_bytes_per_step": down, "steps": E, "ms_per_step": e2e_job_ms / E,
+                    "api": "orb_deposit_host (pinned host SoA in, host grids out)",
+                    "gpu_launches": launches_e},
+            "gpu_launches": launches,
+            "clocks": sampler.summary(),
+            "checks": {"charge_conservation_rel": conservation,
+                       "e2e_charge_conservation_rel": e2e_conservation},
+        }
+        if world == 1 and not args.no_cpu_baseline:
+            n_sample = min(args.cpu_sample, n)
+            npts_o, secs = oracle_sample(cfg, m, n_sample)
+            line["cpu_baseline"] = {
+                "value": npts_o / secs, "unit": UNIT, "cores": 1, "kind": "oracle",
+                "sample": "first %d markers of %s (%d Larmor points, %.1f s), single thread; host has %d cores"
+                          % (n_sample, cfg.name, npts_o, secs, os.cpu_count() or 0)}
+        else:
+            line["cpu_baseline"] = None
+        print(json.dumps(line), flush=True)
+    R.finalize()
+    return 0
+
+
+def main(argv=None):
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default="cfg3", choices=sorted(W.CONFIGS))
+    ap.add_argument("--e2e-steps", type=int, default=3)
+    ap.add_argument("--cpu-sample", type=int, default=1 << 21,
+                    help="markers of the workload the cpu_baseline leg times the oracle on")
+    ap.add_argument("--ref-sample", type=int, default=1 << 18,
+                    help="markers per step of the --impl reference arm")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args(argv)
+    if args.warmup < 3 and args.impl == "ours":
+        print("bench.py: note: fewer than 3 warm-up steps requested", file=sys.stderr)
+    if args.impl == "reference":
+        return run_reference(args)
+    return run_ours(args)
+
+
+if __name__ == "__main__":
+    sys.exit(main())

@@ -140,6 +140,11 @@ int orb_markers_bin(orb_grid_t *g, void *stream);
 int orb_deposit(orb_grid_t *g, double *rho, double *jpar, const orb_nl_policy_t *policy,
                 void *stream);
 
+/* Zeroes rho and, if not NULL, jpar (DEVICE arrays of orb_grid_shape doubles) on `stream`
+ * (two cudaMemsetAsync; no kernel).  Equivalent to ORB_DEPOSIT_ZERO_FIRST, offered as a call of
+ * its own so that a harness can time the deposit kernels apart from the zeroing. */
+int orb_grid_zero(orb_grid_t *g, double *rho, double *jpar, void *stream);
+
 /* Sum of N_L over the markers of the last orb_deposit on this handle.
  * Synchronises with that deposit (one 8-byte device-to-host copy). */
 int orb_last_points(orb_grid_t *g, int64_t *n_points);

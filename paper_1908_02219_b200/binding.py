@@ -21,7 +21,7 @@ ORB_MAX_NL = 32
 
 # every symbol include/orb.h declares
 SYMBOLS = ("orb_grid_create", "orb_grid_destroy", "orb_grid_shape", "orb_markers_bind",
-           "orb_markers_bin", "orb_deposit", "orb_last_points", "orb_deposit_host",
+           "orb_markers_bin", "orb_deposit", "orb_grid_zero", "orb_last_points", "orb_deposit_host",
            "orb_launch_count", "orb_strerror", "orb_last_error", "orb_version")
 
 
@@ -62,6 +62,7 @@ def lib():
     L.orb_markers_bind.argtypes = [vp, C.c_int64, dp, dp, dp, dp, dp, dp, C.c_uint32]
     L.orb_markers_bin.argtypes = [vp, vp]
     L.orb_deposit.argtypes = [vp, dp, dp, C.POINTER(NlPolicy), vp]
+    L.orb_grid_zero.argtypes = [vp, dp, dp, vp]
     L.orb_last_points.argtypes = [vp, i64p]
     L.orb_deposit_host.argtypes = [vp, C.c_int64, dp, dp, dp, dp, dp, dp, dp, dp,
                                    C.POINTER(NlPolicy), i64p, i64p, i64p]
@@ -128,6 +129,9 @@ class Grid:
 
     def deposit(self, rho, jpar, pol: NlPolicy, stream=None):
         _check(lib().orb_deposit(self._h, _ptr(rho), _ptr(jpar), C.byref(pol), stream), self._h)
+
+    def grid_zero(self, rho, jpar, stream=None):
+        _check(lib().orb_grid_zero(self._h, _ptr(rho), _ptr(jpar), stream), self._h)
 
     def last_points(self) -> int:
         v = C.c_int64()

@@ -333,6 +333,17 @@ int orb_deposit(orb_grid_t* g, double* rho, double* jpar, const orb_nl_policy_t*
   return ORB_OK;
 }
 
+int orb_grid_zero(orb_grid_t* g, double* rho, double* jpar, void* stream) {
+  if (!g) return ORB_E_INVAL;
+  if (!rho) return fail(g, ORB_E_INVAL, "rho is NULL");
+  DeviceGuard dg(g->desc.device);
+  if (!dg.ok) return fail(g, ORB_E_CUDA, "cudaSetDevice");
+  cudaStream_t st = static_cast<cudaStream_t>(stream);
+  ORB_CUDA(g, cudaMemsetAsync(rho, 0, (size_t)g->nnodes * sizeof(double), st));
+  if (jpar) ORB_CUDA(g, cudaMemsetAsync(jpar, 0, (size_t)g->nnodes * sizeof(double), st));
+  return ORB_OK;
+}
+
 int orb_last_points(orb_grid_t* g, int64_t* n_points) {
   if (!g || !n_points) return ORB_E_INVAL;
   DeviceGuard dg(g->desc.device);
