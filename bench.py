@@ -237,6 +237,7 @@ def run_ours(args):
         step()
     torch.cuda.synchronize()
     npts_step = g.last_points()
+    fallback_step = g.last_fallback_points()
 
     K = args.steps
     evs = [[torch.cuda.Event(enable_timing=True) for _ in range(4)] for _ in range(K)]
@@ -310,6 +311,7 @@ def run_ours(args):
             "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
             "config": config_json(cfg, world),
             "points_per_step": npts_step,
+            "fallback_points_per_step": fallback_step,
             "phases_ms": {"bin": bin_ms, "zero": zero_ms, "deposit": dep_ms,
                           "deposit_min": min(dep_ms_all), "deposit_max": max(dep_ms_all)},
             "deposit_only": {"value": npts_step / (dep_ms * 1e-3), "unit": UNIT,

@@ -149,6 +149,12 @@ int orb_grid_zero(orb_grid_t *g, double *rho, double *jpar, void *stream);
  * Synchronises with that deposit (one 8-byte device-to-host copy). */
 int orb_last_points(orb_grid_t *g, int64_t *n_points);
 
+/* Of those, the Larmor points of the last orb_deposit whose 4x4 (s, theta*) footprint left the
+ * shared-memory tile of their block and were deposited with global atomics instead (a
+ * performance diagnostic; 0 for the global-atomics algorithm).  Synchronises like
+ * orb_last_points. */
+int orb_last_fallback_points(orb_grid_t *g, int64_t *n_points);
+
 /* End-to-end convenience for callers whose data lives on the HOST: copies the six
  * marker arrays (host pointers, n doubles each; vpar may be NULL iff jpar_host is
  * NULL) to library-owned device buffers, binds, deposits into zeroed device grids

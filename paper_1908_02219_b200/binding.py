@@ -21,7 +21,7 @@ ORB_MAX_NL = 32
 
 # every symbol include/orb.h declares
 SYMBOLS = ("orb_grid_create", "orb_grid_destroy", "orb_grid_shape", "orb_markers_bind",
-           "orb_markers_bin", "orb_deposit", "orb_grid_zero", "orb_last_points", "orb_deposit_host",
+           "orb_markers_bin", "orb_deposit", "orb_grid_zero", "orb_last_points", "orb_last_fallback_points", "orb_deposit_host",
            "orb_launch_count", "orb_strerror", "orb_last_error", "orb_version")
 
 
@@ -64,6 +64,7 @@ def lib():
     L.orb_deposit.argtypes = [vp, dp, dp, C.POINTER(NlPolicy), vp]
     L.orb_grid_zero.argtypes = [vp, dp, dp, vp]
     L.orb_last_points.argtypes = [vp, i64p]
+    L.orb_last_fallback_points.argtypes = [vp, i64p]
     L.orb_deposit_host.argtypes = [vp, C.c_int64, dp, dp, dp, dp, dp, dp, dp, dp,
                                    C.POINTER(NlPolicy), i64p, i64p, i64p]
     L.orb_launch_count.argtypes = [vp, i64p]
@@ -136,6 +137,11 @@ class Grid:
     def last_points(self) -> int:
         v = C.c_int64()
         _check(lib().orb_last_points(self._h, C.byref(v)), self._h)
+        return v.value
+
+    def last_fallback_points(self) -> int:
+        v = C.c_int64()
+        _check(lib().orb_last_fallback_points(self._h, C.byref(v)), self._h)
         return v.value
 
     def launch_count(self) -> int:

@@ -217,8 +217,8 @@ int orb_grid_create(const orb_grid_desc_t* d, orb_grid_t** out) {
   g->bin.ncells = ncells;
   const int total = ORB_MAX_NL * (ORB_MAX_NL + 1) / 2;
   if (cudaMalloc(&g->ring, total * sizeof(double2)) != cudaSuccess ||
-      cudaMalloc(&g->d_points, sizeof(unsigned long long)) != cudaSuccess ||
-      cudaMemset(g->d_points, 0, sizeof(unsigned long long)) != cudaSuccess) {
+      cudaMalloc(&g->d_points, 2 * sizeof(unsigned long long)) != cudaSuccess ||
+      cudaMemset(g->d_points, 0, 2 * sizeof(unsigned long long)) != cudaSuccess) {
     cudaGetLastError();
     cudaFree(g->ring);
     cudaFree(g->d_points);
@@ -314,7 +314,7 @@ int orb_deposit(orb_grid_t* g, double* rho, double* jpar, const orb_nl_policy_t*
     ORB_CUDA(g, cudaMemsetAsync(rho, 0, (size_t)g->nnodes * sizeof(double), st));
     if (jpar) ORB_CUDA(g, cudaMemsetAsync(jpar, 0, (size_t)g->nnodes * sizeof(double), st));
   }
-  ORB_CUDA(g, cudaMemsetAsync(g->d_points, 0, sizeof(unsigned long long), st));
+  ORB_CUDA(g, cudaMemsetAsync(g->d_points, 0, 2 * sizeof(unsigned long long), st));
 
   Params P = make_params(g, pol);
   Markers M = g->bound;
@@ -351,6 +351,16 @@ int orb_last_points(orb_grid_t* g, int64_t* n_points) {
   // default-stream copy: waits for prior work on blocking streams; then make sure
   ORB_CUDA(g, cudaDeviceSynchronize());
   ORB_CUDA(g, cudaMemcpy(&v, g->d_points, sizeof(v), cudaMemcpyDeviceToHost));
+  *n_points = (int64_t)v;
+  return ORB_OK;
+}
+
+int orb_last_fallback_points(orb_grid_t* g, int64_t* n_points) {
+  if (!g || !n_points) return ORB_E_INVAL;
+  DeviceGuard dg(g->desc.device);
+  unsigned long long v = 0;
+  ORB_CUDA(g, cudaDeviceSynchronize());
+  ORB_CUDA(g, cudaMemcpy(&v, g->d_points + 1, sizeof(v), cudaMemcpyDeviceToHost));
   *n_points = (int64_t)v;
   return ORB_OK;
 }
