@@ -170,6 +170,12 @@ int orb_deposit_host(orb_grid_t *g, int64_t n, const double *s, const double *th
  * (memsets and copies not counted). */
 int orb_launch_count(const orb_grid_t *g, int64_t *n_launches);
 
+/* Host-only diagnostic, no device needed: the polynomial pieces of the clamped (open knot
+ * vector) radial cubic B-splines that the tile kernel evaluates (R11).
+ * out (HOST, ns*16 doubles): out[(c*4 + a)*4 + d] = coefficient of t^d, t = s*ns - c in [0,1),
+ * of basis function c+a on radial cell c.  ORB_E_INVAL if ns < 4 or out is NULL. */
+int orb_spline_table_radial(int32_t ns, double *out);
+
 /* Static text for a status code. */
 const char *orb_strerror(int code);
 

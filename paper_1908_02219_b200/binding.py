@@ -22,7 +22,7 @@ ORB_MAX_NL = 32
 # every symbol include/orb.h declares
 SYMBOLS = ("orb_grid_create", "orb_grid_destroy", "orb_grid_shape", "orb_markers_bind",
            "orb_markers_bin", "orb_deposit", "orb_grid_zero", "orb_last_points", "orb_last_fallback_points", "orb_deposit_host",
-           "orb_launch_count", "orb_strerror", "orb_last_error", "orb_version")
+           "orb_launch_count", "orb_spline_table_radial", "orb_strerror", "orb_last_error", "orb_version")
 
 
 class OrbError(RuntimeError):
@@ -68,6 +68,7 @@ def lib():
     L.orb_deposit_host.argtypes = [vp, C.c_int64, dp, dp, dp, dp, dp, dp, dp, dp,
                                    C.POINTER(NlPolicy), i64p, i64p, i64p]
     L.orb_launch_count.argtypes = [vp, i64p]
+    L.orb_spline_table_radial.argtypes = [C.c_int32, dp]
     L.orb_strerror.argtypes = [C.c_int]
     L.orb_strerror.restype = C.c_char_p
     L.orb_last_error.argtypes = [vp]
@@ -101,6 +102,14 @@ def _ptr(t):
 def policy(n_fixed=4, *, adaptive=False, n_max=None, rho_ref=1.0, alpha0=0.0, flags=0) -> NlPolicy:
     return NlPolicy(ORB_NL_ADAPTIVE if adaptive else ORB_NL_FIXED, n_fixed,
                     n_max if n_max is not None else n_fixed, flags, rho_ref, alpha0)
+
+
+def spline_table_radial(ns: int):
+    """(ns, 4, 4) numpy array: [cell, basis offset a, power of t] (host-only diagnostic)."""
+    import numpy as np
+    out = np.empty((ns, 4, 4), dtype=np.float64)
+    _check(lib().orb_spline_table_radial(ns, out.ctypes.data))
+    return out
 
 
 class Grid:

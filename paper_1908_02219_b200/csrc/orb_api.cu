@@ -25,6 +25,7 @@ struct orb_grid {
   // scratch (owned)
   BinScratch bin;
   int64_t bin_capacity;      // markers the rank/rec buffers can hold
+  double* scoef;             // device table of the radial spline pieces (ns*16 doubles)
   double2* ring;             // device ring table
   double ring_alpha0;
   bool ring_valid;
@@ -98,6 +99,7 @@ Params make_params(const orb_grid* g, const orb_nl_policy_t* pol) {
     P.rho_ref = P.adaptive ? pol->rho_ref : 1.0;
   }
   P.ring = g->ring;
+  P.scoef = g->scoef;
   return P;
 }
 
@@ -216,10 +218,16 @@ int orb_grid_create(const orb_grid_desc_t* d, orb_grid_t** out) {
   g->nnodes = nnodes;
   g->bin.ncells = ncells;
   const int total = ORB_MAX_NL * (ORB_MAX_NL + 1) / 2;
-  if (cudaMalloc(&g->ring, total * sizeof(double2)) != cudaSuccess ||
+  std::vector<double> table;
+  build_radial_table(d->ns, table);
+  if (cudaMalloc(&g->scoef, table.size() * sizeof(double)) != cudaSuccess ||
+      cudaMemcpy(g->scoef, table.data(), table.size() * sizeof(double), cudaMemcpyHostToDevice) !=
+          cudaSuccess ||
+      cudaMalloc(&g->ring, total * sizeof(double2)) != cudaSuccess ||
       cudaMalloc(&g->d_points, 2 * sizeof(unsigned long long)) != cudaSuccess ||
       cudaMemset(g->d_points, 0, 2 * sizeof(unsigned long long)) != cudaSuccess) {
     cudaGetLastError();
+    cudaFree(g->scoef);
     cudaFree(g->ring);
     cudaFree(g->d_points);
     delete g;
@@ -236,6 +244,7 @@ int orb_grid_destroy(orb_grid_t* g) {
   free_bin(g);
   cudaFree(g->bin.cell_start);
   cudaFree(g->bin.block_sums);
+  cudaFree(g->scoef);
   cudaFree(g->ring);
   cudaFree(g->d_points);
   for (int i = 0; i < 6; ++i) cudaFree(g->hbuf[i]);
@@ -243,6 +252,14 @@ int orb_grid_destroy(orb_grid_t* g) {
   cudaFree(g->hgrid[1]);
   cudaGetLastError();
   delete g;
+  return ORB_OK;
+}
+
+int orb_spline_table_radial(int32_t ns, double* out) {
+  if (ns < 4 || !out) return ORB_E_INVAL;
+  std::vector<double> table;
+  build_radial_table(ns, table);
+  memcpy(out, table.data(), table.size() * sizeof(double));
   return ORB_OK;
 }
 

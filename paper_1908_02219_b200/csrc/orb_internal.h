@@ -4,6 +4,8 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 
+#include <vector>
+
 #include "orb.h"
 
 namespace orb {
@@ -29,6 +31,9 @@ struct Params {
   double rho_ref;
   // ring table: entry (N, l) at N*(N-1)/2 + l holds (cos, sin)(alpha0 + 2 pi l / N), N = 1..ORB_MAX_NL
   const double2* ring;
+  // radial spline pieces: scoef[(c*4 + a)*4 + d] = coefficient of t^d of basis c+a on cell c
+  // (orb_spline_table.cu)
+  const double* scoef;
 };
 
 // Bound markers: either the caller's SoA arrays (in bound order) or the library's
@@ -60,5 +65,8 @@ int launch_bin(const Params& P, const Markers& M, const BinScratch& B, bool pres
 
 int launch_deposit_tile(const Params& P, const Markers& M, const uint32_t* cell_start, double* rho,
                         double* jpar, unsigned long long* d_points, cudaStream_t st);
+
+// host: polynomial pieces of the clamped radial cubic B-splines, ns*16 doubles
+void build_radial_table(int ns, std::vector<double>& out);
 
 }  // namespace orb

@@ -77,3 +77,32 @@ def test_product_does_not_import_oracle():
                 text = open(os.path.join(dirpath, f)).read()
                 assert not re.search(r"^\s*(import|from)\s+oracle\b", text, flags=re.M), f
                 assert "orb_oracle" not in text and "liborb_oracle" not in text, f
+
+
+@pytest.mark.parametrize("ns", [4, 5, 7, 16, 128])
+def test_radial_spline_table_matches_scipy(L, ns):
+    """Host logic of the tile kernel: the polynomial pieces of the clamped cubic B-splines
+    (orb_spline_table_radial) evaluated by Horner equal scipy's BSpline design matrix on the same
+    open knot vector, in every cell including the four end cells; and they sum to one."""
+    import numpy as np
+    from scipy import interpolate
+    tab = B.spline_table_radial(ns)
+    assert tab.shape == (ns, 4, 4)
+    T = np.array([0.0] * 3 + list(range(ns + 1)) + [float(ns)] * 3)
+    rng = np.random.default_rng(ns)
+    for c in list(range(min(ns, 4))) + list(range(max(ns - 4, 0), ns)) + [ns // 2]:
+        for t in list(rng.uniform(0, 1, 8)) + [0.0, 0.5, 1.0 - 1e-12]:
+            x = c + t
+            t = x - c   # the in-cell coordinate scipy actually sees
+            row = interpolate.BSpline.design_matrix(np.array([min(x, ns)]), T, 3).toarray()[0]
+            got = np.zeros(ns + 3)
+            for a in range(4):
+                k = tab[c, a]
+                got[c + a] = ((k[3] * t + k[2]) * t + k[1]) * t + k[0]
+            np.testing.assert_allclose(got, row, rtol=0, atol=5e-15)
+            assert abs(got.sum() - 1.0) < 5e-15
+    # interior cells hold the cardinal pieces exactly
+    if ns >= 8:
+        want = np.array([[1 / 6, -0.5, 0.5, -1 / 6], [2 / 3, 0, -1, 0.5], [1 / 6, 0.5, 0.5, -0.5],
+                         [0, 0, 0, 1 / 6]])
+        np.testing.assert_allclose(tab[ns // 2], want, rtol=0, atol=1e-15)
