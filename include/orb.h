@@ -166,6 +166,11 @@ int orb_deposit_host(orb_grid_t *g, int64_t n, const double *s, const double *th
                      double *rho_host, double *jpar_host, const orb_nl_policy_t *policy,
                      int64_t *n_points, int64_t *h2d_bytes, int64_t *d2h_bytes);
 
+/* Diagnostic: the 16 device counters of the last orb_deposit.  out[0] = Larmor points,
+ * out[1] = points deposited directly; out[2..15] = per-phase SM clock sums of the tile kernel
+ * (block-thread 0), non-zero only in a library built with -DORB_PHASE_CLOCKS.  Synchronises. */
+int orb_debug_counters(orb_grid_t *g, uint64_t out[16]);
+
 /* Number of kernel launches the library has enqueued on this handle so far
  * (memsets and copies not counted). */
 int orb_launch_count(const orb_grid_t *g, int64_t *n_launches);

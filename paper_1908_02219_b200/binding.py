@@ -22,7 +22,7 @@ ORB_MAX_NL = 32
 # every symbol include/orb.h declares
 SYMBOLS = ("orb_grid_create", "orb_grid_destroy", "orb_grid_shape", "orb_markers_bind",
            "orb_markers_bin", "orb_deposit", "orb_grid_zero", "orb_last_points", "orb_last_fallback_points", "orb_deposit_host",
-           "orb_launch_count", "orb_spline_table_radial", "orb_strerror", "orb_last_error", "orb_version")
+           "orb_launch_count", "orb_debug_counters", "orb_spline_table_radial", "orb_strerror", "orb_last_error", "orb_version")
 
 
 class OrbError(RuntimeError):
@@ -152,6 +152,11 @@ class Grid:
         v = C.c_int64()
         _check(lib().orb_last_fallback_points(self._h, C.byref(v)), self._h)
         return v.value
+
+    def debug_counters(self):
+        out = (C.c_uint64 * 16)()
+        _check(lib().orb_debug_counters(self._h, out), self._h)
+        return list(out)
 
     def launch_count(self) -> int:
         v = C.c_int64()

@@ -224,8 +224,8 @@ int orb_grid_create(const orb_grid_desc_t* d, orb_grid_t** out) {
       cudaMemcpy(g->scoef, table.data(), table.size() * sizeof(double), cudaMemcpyHostToDevice) !=
           cudaSuccess ||
       cudaMalloc(&g->ring, total * sizeof(double2)) != cudaSuccess ||
-      cudaMalloc(&g->d_points, 2 * sizeof(unsigned long long)) != cudaSuccess ||
-      cudaMemset(g->d_points, 0, 2 * sizeof(unsigned long long)) != cudaSuccess) {
+      cudaMalloc(&g->d_points, kCounters * sizeof(unsigned long long)) != cudaSuccess ||
+      cudaMemset(g->d_points, 0, kCounters * sizeof(unsigned long long)) != cudaSuccess) {
     cudaGetLastError();
     cudaFree(g->scoef);
     cudaFree(g->ring);
@@ -331,7 +331,7 @@ int orb_deposit(orb_grid_t* g, double* rho, double* jpar, const orb_nl_policy_t*
     ORB_CUDA(g, cudaMemsetAsync(rho, 0, (size_t)g->nnodes * sizeof(double), st));
     if (jpar) ORB_CUDA(g, cudaMemsetAsync(jpar, 0, (size_t)g->nnodes * sizeof(double), st));
   }
-  ORB_CUDA(g, cudaMemsetAsync(g->d_points, 0, 2 * sizeof(unsigned long long), st));
+  ORB_CUDA(g, cudaMemsetAsync(g->d_points, 0, kCounters * sizeof(unsigned long long), st));
 
   Params P = make_params(g, pol);
   Markers M = g->bound;
@@ -379,6 +379,15 @@ int orb_last_fallback_points(orb_grid_t* g, int64_t* n_points) {
   ORB_CUDA(g, cudaDeviceSynchronize());
   ORB_CUDA(g, cudaMemcpy(&v, g->d_points + 1, sizeof(v), cudaMemcpyDeviceToHost));
   *n_points = (int64_t)v;
+  return ORB_OK;
+}
+
+int orb_debug_counters(orb_grid_t* g, uint64_t out[16]) {
+  if (!g || !out) return ORB_E_INVAL;
+  DeviceGuard dg(g->desc.device);
+  ORB_CUDA(g, cudaDeviceSynchronize());
+  ORB_CUDA(g, cudaMemcpy(out, g->d_points, kCounters * sizeof(unsigned long long),
+                         cudaMemcpyDeviceToHost));
   return ORB_OK;
 }
 

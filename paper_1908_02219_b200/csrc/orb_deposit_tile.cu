@@ -1,39 +1,50 @@
-// Tile deposition, v2 (hot-path steps a1-a6, a8, a9): register accumulation through the fp64
-// MMA unit, no shared-memory atomics on the per-point path.
+// Tile deposition, v3 (hot-path steps a1-a6, a8, a9): register accumulation through the fp64
+// MMA unit; no atomics of any kind on the per-point path.
 //
 // One thread block per grid tile = (1 toroidal cell slab k) x (kTileI radial cells) x (kTileJ
 // poloidal cells); its markers are found through the binning pass's per-cell offsets
 // (orb_bin.cu; key phi-major, so every radial row of the tile is one contiguous run).  The tile's
-// markers are processed in chunks of <= kPCap Larmor points; per chunk
+// markers are processed in chunks of <= kPCap Larmor points (a cfg3 tile is one chunk); per chunk
 //
-//   phase 1  (one lane per marker, then one lane per Larmor point -- the ring expansion is
-//            warp-cooperative so that adaptive N_L = 4..32 keeps every lane busy):
-//            marker -> guiding-centre geometry, N_L, c = q w / N_L, c * phi-weights, v_par
-//            (a 40-byte entry of a shared-memory marker table);  Larmor point -> (s_l, theta*_l)
-//            -> (s, theta*) cell + in-cell coordinates (t_s, t_theta), appended as a 16-byte
-//            record; a per-cell counter is bumped (native 32-bit shared atomics).
-//   phase 1c exclusive scan of the per-cell counts and an index permutation: the chunk's points
-//            are now grouped by (s, theta*) cell.  (This is the paper's "sorting Larmor points by
+//   phase 1a (one lane per marker): marker -> guiding-centre geometry, N_L, c = q w / N_L,
+//            c * phi-weights, v_par into a shared-memory marker table; a prefix sum of N_L over
+//            the warp's 32 markers allocates the slots of their Larmor points.
+//   phase 1b (one lane per Larmor point, all threads, evenly -- adaptive N_L = 4..32 keeps every
+//            lane busy): point -> (s_l, theta*_l) -> (s, theta*) cell + in-cell coordinates
+//            (t_s, t_theta), a 16-byte record; a per-cell counter is bumped (native 32-bit shared
+//            atomic) and its return value is the point's rank inside its cell.
+//   phase 1c exclusive scan of the per-cell counts, each rounded up to a multiple of 4, and an
+//            index permutation: the chunk's points are now grouped by (s, theta*) cell, padded
+//            with a zero-weight dummy point.  (This is the paper's "sorting Larmor points by
 //            cell", done per tile in shared memory instead of in HBM.)
-//   phase 2  warps walk rows of cells along theta*.  All points of one cell hit the same 4 x 4
-//            (s, theta*) nodes x 4 phi planes x {rho, jpar}; their sum is the dense contraction
+//   phase 2  each warp owns a row segment of kSegW cells and walks it along theta*.  All points of
+//            one cell hit the same 4 x 4 (s, theta*) nodes x 4 phi planes x {rho, jpar}; their sum
+//            is the dense contraction
 //                 C[node(a,b)][channel(d,grid)] = sum_pts  ws_a(pt) wt_b(pt) * cw_d(pt) {1, vpar(pt)}
 //            = A (16 x npts) . B (npts x 8), issued as two DMMA m8n8k4 per 4 points with the
-//            accumulators in registers.  Each lane prepares ONE spline value per step (a cubic in
-//            t with lane-constant coefficients, 3 FMA), the operands are exchanged by shuffles.
-//            Stepping to the next cell shifts the accumulators by one node column (shuffle) and
-//            retires the column that can receive nothing more into the shared-memory tile.
+//            accumulators in registers.  Each lane prepares ONE spline value per batch (a cubic in
+//            t with lane-constant coefficients, 3 FMA); operands are exchanged by shuffles.  The
+//            four node columns of the accumulator window live in four fixed "slots" (half-warp x
+//            DMMA); stepping to the next cell retires the slot of the finished column with one
+//            128-bit store per lane of a half-warp and re-uses it for the new column -- no data
+//            moves, only the shuffle source lanes rotate (the walk is unrolled by 4).
+//            Retired columns go to partial[row segment][node column][a][channel]: the radial
+//            offset a is kept apart, so every entry has exactly one writer and is written once
+//            per chunk -- plain stores, no read-modify-write, no atomics.
 //
-// and at the end the tile (nodes incl. halo x 4 planes x {rho, jpar}) is flushed ONCE with fp64
-// RED.ADD to global memory.  Points whose cell leaves the tile's halo (long rings, rounding at a
-// slab boundary) are deposited directly with global atomics (rare; counted).
+// and at the end the tile's nodes are summed from the partial array (4 radial offsets, 2
+// overlapping segments) and flushed ONCE with fp64 RED.ADD to global memory.  Points whose cell
+// leaves the tile's halo (long rings, rounding at a slab boundary) are deposited directly with
+// global atomics (rare; counted).
 //
 // Why this shape: profiles/r01_microbench.md -- shared-memory fp64 atomics are CAS loops
 // (1.5 updates/clk/SM at this access pattern) and global fp64 REDs issue at 0.78 lanes/clk/SM,
 // while the path needs 128 node updates per Larmor point; only register accumulators keep up with
 // the fp64 pipe (64 FMA/clk/SM).  DMMA runs on that same pipe at the same FMA rate (measured
 // 18.5 TFMA/s either way) but needs one operand pair per 8 FMAs, which is what makes the operand
-// traffic fit.
+// traffic fit.  profiles/r01_v2_deposit_ncu.md -- v2 spent 38 warp instructions per point, 58 % of
+// them in phase 2 (window shift by shuffles, CAS retire loops); v3's slot rotation and
+// single-writer partial array remove both.
 #include "orb_geom.cuh"
 
 namespace orb {
@@ -43,35 +54,50 @@ namespace {
 constexpr int kThreads = 512;
 constexpr int kWarps = kThreads / 32;
 constexpr int kTileI = 8;     // radial cells per tile
-constexpr int kTileJ = 32;    // poloidal cells per tile
+constexpr int kTileJ = 16;    // poloidal cells per tile
 constexpr int kHaloS = 2;     // ring reach in s covered by the tile, cells
 constexpr int kHaloT = 4;     // ring reach in theta* covered by the tile, cells
 constexpr int kCH = kTileI + 2 * kHaloS;   // cell rows held (12)
-constexpr int kCW = kTileJ + 2 * kHaloT;   // cell columns held (40)
+constexpr int kCW = kTileJ + 2 * kHaloT;   // cell columns held (24)
 constexpr int kNH = kCH + 3;               // node rows (15)
-constexpr int kNW = kCW + 3;               // node columns (43)
-constexpr int kCells = kCH * kCW;
-constexpr int kPCap = 4096;   // Larmor points per chunk
-constexpr int kMCap = 1024;   // markers per chunk
-constexpr int kSegW = 10;     // cells per walk segment
-constexpr int kSegs = kCW / kSegW;
-constexpr int kItems = kCH * kSegs;
+constexpr int kNW = kCW + 3;               // node columns (27)
+constexpr int kCells = kCH * kCW;          // 288
+constexpr int kSegW = 12;                  // cells per walk segment
+constexpr int kSegs = kCW / kSegW;         // 2
+constexpr int kSegN = kSegW + 3;           // node columns a segment produces (15)
+constexpr int kItems = kCH * kSegs;        // 24
+constexpr int kPCap = 3072;   // Larmor points per chunk
+constexpr int kMCap = 768;    // markers per chunk
+constexpr int kPermCap = ((kPCap + 3 * kCells + 3) / 4) * 4;   // points + padding to batches of 4
 constexpr unsigned kFull = 0xffffffffu;
-constexpr unsigned short kNoCell = 0xffffu;
-static_assert(kCW % kSegW == 0, "segments must tile the row");
-static_assert(kPCap >= 32 * ORB_MAX_NL && kPCap <= 65535 && kMCap <= 65535 && kMCap % 32 == 0, "caps");
-static_assert(kCells < kNoCell, "cell id must fit 16 bits");
+constexpr unsigned kNoCell = 0x1ffu;       // meta cell field of a point deposited directly
+static_assert(kCW % kSegW == 0 && kSegW % 4 == 0, "segments must tile the row in groups of 4");
+static_assert(kPCap >= 32 * ORB_MAX_NL && kPCap < 4096 && kMCap % 32 == 0 && kMCap < 2047, "caps");
+static_assert(kCells < (int)kNoCell, "cell id must fit 9 bits");
+
+// meta word of a point slot.  After phase 1a: marker slot << 21 | point index in the ring.
+// After phase 1b: marker slot << 21 | rank inside the cell << 9 | tile-local cell.
+__device__ __forceinline__ unsigned meta_marker(unsigned m) { return m >> 21; }
+
+struct MarkerTmp {      // phase 1a -> 1b hand-over, 32 bytes
+  double a, b;          // (x0, z0), or (s, theta*) when N_L = 1
+  double rho;
+  int n;                // N_L; bit 8 set if the marker's phi cell is not this block's slab
+  int k0;               // first phi node (phi cell - 1)
+};
 
 template <int G>
 struct Smem {
-  double tile[kNH * kNW * 4 * G];     // [node row][node col][grid][phi plane]
-  double2 rec[kPCap];                 // (t_s, t_theta) of a Larmor point
-  double mtab[kMCap * 5];             // per marker: c*wphi[0..3], vpar
-  unsigned short pmark[kPCap];        // marker-table slot of a point
-  unsigned short pcell[kPCap];        // tile-local cell of a point, kNoCell if deposited directly
-  unsigned short perm[kPCap];         // points grouped by cell
-  unsigned int count[kCells + 1];     // per-cell counts, then running cursors
-  unsigned int cstart[kCells + 1];    // exclusive scan of count
+  double partial[kItems * kSegN * 32];   // [row segment][node col][a][grid*4 + phi plane]
+  double2 rec[kPCap + 1];                // (t_s, t_theta) of a Larmor point; [kPCap] = dummy
+  double mtab[(kMCap + 1) * 5];          // per marker: c*wphi[0..3], vpar; [kMCap] = dummy (zeros)
+  union {
+    MarkerTmp mtmp[kMCap];               // phases 1a-1b
+    unsigned int perm[kPermCap];         // phases 1c-2: points grouped by cell, each cell padded
+  };                                     // to 4; entry = point slot | marker slot << 16
+  unsigned int meta[kPCap + 1];
+  unsigned int count[kCells + 1];        // per-cell counts
+  unsigned int cstart[kCells + 1];       // exclusive scan of the padded counts
   unsigned int row_begin[kTileI], row_off[kTileI + 1];
   int deferred[2][kWarps];
   int n_deferred[2];
@@ -82,8 +108,21 @@ struct Smem {
   int next_item;
 };
 
+#ifdef ORB_PHASE_CLOCKS
+#define ORB_CLK(i)                                                          \
+  do {                                                                      \
+    if (tid == 0) {                                                         \
+      const long long now__ = clock64();                                    \
+      atomicAdd(d_points + 2 + (i), (unsigned long long)(now__ - clk__));   \
+      clk__ = now__;                                                        \
+    }                                                                       \
+  } while (0)
+#else
+#define ORB_CLK(i) do { } while (0)
+#endif
+
 __device__ __forceinline__ void dmma884(double& c0, double& c1, double a, double b) {
-  asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};"
+  asm("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};"
                : "+d"(c0), "+d"(c1)
                : "d"(a), "d"(b));
 }
@@ -129,14 +168,14 @@ __global__ void __launch_bounds__(kThreads, 1)
 k_deposit_tile(const Params P, const Markers M, const uint32_t* __restrict__ cell_start,
                double* __restrict__ rho, double* __restrict__ jpar,
                unsigned long long* __restrict__ d_points, int tiles_i, int tiles_j) {
-  constexpr int NC = 4 * G;   // channels per (s, theta*) node: channel = grid*4 + phi plane
   extern __shared__ __align__(16) unsigned char smem_raw[];
   Smem<G>& S = *reinterpret_cast<Smem<G>*>(smem_raw);
 
   const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
-  const int tj = blockIdx.x % tiles_j;
-  const int ti = (blockIdx.x / tiles_j) % tiles_i;
-  const int k = blockIdx.x / (tiles_j * tiles_i);
+#ifdef ORB_PHASE_CLOCKS
+  long long clk__ = clock64();
+#endif
+  const int tj = blockIdx.x, ti = blockIdx.y, k = blockIdx.z;
   const int i_lo = ti * kTileI, j_lo = tj * kTileJ;
   const int i_hi = min(i_lo + kTileI, P.ns), j_hi = min(j_lo + kTileJ, P.nth);
   const int row_base = i_lo - kHaloS;        // radial cell (= first basis index) of cell row 0
@@ -164,21 +203,27 @@ k_deposit_tile(const Params P, const Markers M, const uint32_t* __restrict__ cel
     S.pts_end = 0xffffffffu;
     S.full = 0;
     S.next_item = 0;
+    // dummy point and dummy marker used to pad every cell's point list to a multiple of 4
+    S.rec[kPCap] = make_double2(0.0, 0.0);
+    S.meta[kPCap] = (unsigned)kMCap << 21;
+#pragma unroll
+    for (int d = 0; d < 5; ++d) S.mtab[kMCap * 5 + d] = 0.0;
   }
   __syncthreads();
   const uint32_t n_tile = S.row_off[kTileI];
   if (n_tile == 0) return;
   const int n_groups = (int)((n_tile + 31) / 32);
 
-  for (int x = tid; x < kNH * kNW * NC; x += kThreads) S.tile[x] = 0.0;
   for (int x = tid; x <= kCells; x += kThreads) S.count[x] = 0;
   __syncthreads();
 
+  ORB_CLK(0);   // prologue
   unsigned int my_points = 0, my_fallback = 0;
-  int cur = 0;   // which deferred list is being consumed this chunk
+  int cur = 0;     // which deferred list is being consumed this chunk
+  int chunk = 0;
 
   for (;;) {
-    // ------------------------------------------------------------------ phase 1
+    // ------------------------------------------------------------------ phase 1a: markers
     for (;;) {
       int grp = -1;
       if (lane == 0) {
@@ -193,7 +238,6 @@ k_deposit_tile(const Params P, const Markers M, const uint32_t* __restrict__ cel
       grp = __shfl_sync(kFull, grp, 0);
       if (grp < 0) break;
 
-      // a1-a3: one lane per marker
       const uint32_t v = (uint32_t)grp * 32u + (uint32_t)lane;
       const bool have = v < n_tile;
       int n = 0, k0 = 0;
@@ -221,7 +265,8 @@ k_deposit_tile(const Params P, const Markers M, const uint32_t* __restrict__ cel
         }
         grho = g.rho;
       }
-      // the marker was binned into slab k, so k0 == k - 1 up to rounding at a cell boundary
+      // the marker was binned into slab k, so k0 == k - 1 up to rounding at a cell boundary;
+      // if not, its points take the direct path
       const int k_ok = have && (k0 == k - 1);
 
       int incl = n;
@@ -258,87 +303,79 @@ k_deposit_tile(const Params P, const Markers M, const uint32_t* __restrict__ cel
       pb = __shfl_sync(kFull, pb, 0);
       my_points += (unsigned)n;
 
+      const unsigned int ms = mb + (unsigned)lane;
       {
-        double* e = S.mtab + (size_t)(mb + lane) * 5;
+        double* e = S.mtab + (size_t)ms * 5;
         e[0] = cw[0]; e[1] = cw[1]; e[2] = cw[2]; e[3] = cw[3]; e[4] = vpar;
+        MarkerTmp t;
+        t.a = ga; t.b = gb; t.rho = grho;
+        t.n = n | (k_ok ? 0 : 256);
+        t.k0 = k0;
+        S.mtmp[ms] = t;
       }
-      __syncwarp();
-
-      // a4-a6: one lane per Larmor point of the group's 32 markers
-      const int uniform_n = P.adaptive ? 0 : P.n_fixed;
-      for (int q0 = 0; q0 < total; q0 += 32) {
-        const int q = q0 + lane;
-        const bool pvalid = q < total;
-        const int qq = pvalid ? q : total - 1;
-        int owner;
-        if (uniform_n) {
-          owner = qq / uniform_n;
-        } else {
-          owner = 0;
-#pragma unroll
-          for (int step = 16; step >= 1; step >>= 1) {
-            const int t = __shfl_sync(kFull, incl, owner + step - 1);
-            if (t <= qq) owner += step;
-          }
-        }
-        const int o_incl = __shfl_sync(kFull, incl, owner);
-        const int o_n = __shfl_sync(kFull, n, owner);
-        const double o_a = __shfl_sync(kFull, ga, owner);
-        const double o_b = __shfl_sync(kFull, gb, owner);
-        const double o_rho = __shfl_sync(kFull, grho, owner);
-        const int o_kok = __shfl_sync(kFull, k_ok, owner);
-        const int o_k0 = __shfl_sync(kFull, k0, owner);
-        if (!pvalid) continue;
-        const int l = qq - (o_incl - o_n);
-        double s_l, ts_l;
-        if (o_n == 1) {
-          s_l = o_a;
-          ts_l = o_b;
-        } else {
-          GuidingCentre g;
-          g.x0 = o_a;
-          g.z0 = o_b;
-          g.rho = o_rho;
-          larmor_point(P, g, ring_entry(P, o_n, l), s_l, ts_l);
-        }
-        const double xs = s_l * (double)P.ns;
-        const int ci = min((int)xs, P.ns - 1);
-        const double t_s = xs - (double)ci;
-        double t_t;
-        const int cj = periodic_cell(ts_l, P.nth_scale, P.nth, t_t);
-        const int lr = ci - row_base;
-        int lc = cj - cellcol_base;
-        if (lc >= P.nth) lc -= P.nth;
-        if (lc < 0) lc += P.nth;
-        const unsigned int slot = pb + (unsigned)q;
-        if (o_kok && lr >= 0 && lr < kCH && lc >= 0 && lc < kCW) {
-          const int cell = lr * kCW + lc;
-          S.rec[slot] = make_double2(t_s, t_t);
-          S.pmark[slot] = (unsigned short)(mb + owner);
-          S.pcell[slot] = (unsigned short)cell;
-          atomicAdd(&S.count[cell], 1u);
-        } else {
-          // footprint leaves the tile (long ring, or phi rounding): global atomics
-          S.pcell[slot] = kNoCell;
-          ++my_fallback;
-          const double* e = S.mtab + (size_t)(mb + owner) * 5;
-          deposit_point_global<G>(P, s_l, ts_l, o_k0, e, e[4], rho, jpar);
-        }
+      {
+        unsigned int q = pb + (unsigned)(incl - n);
+        const unsigned int hi = ms << 21;
+        for (int l = 0; l < n; ++l) S.meta[q + l] = hi | (unsigned)l;
       }
     }
     __syncthreads();
+    ORB_CLK(1);   // phase 1a
 
-    // ------------------------------------------------------------------ phase 1c
+    // ------------------------------------------------------------------ phase 1b: Larmor points
     const unsigned int n_rec = min(S.npts, S.pts_end);
+    for (unsigned int q = tid; q < n_rec; q += kThreads) {
+      const unsigned int m0 = S.meta[q];
+      const unsigned int ms = meta_marker(m0);
+      const int l = (int)(m0 & 0x1fu);
+      const MarkerTmp mt = S.mtmp[ms];
+      double s_l, ts_l;
+      const int n = mt.n & 255;
+      if (n == 1) {
+        s_l = mt.a;
+        ts_l = mt.b;
+      } else {
+        GuidingCentre g;
+        g.x0 = mt.a;
+        g.z0 = mt.b;
+        g.rho = mt.rho;
+        larmor_point(P, g, ring_entry(P, n, l), s_l, ts_l);
+      }
+      const double xs = s_l * (double)P.ns;
+      const int ci = min((int)xs, P.ns - 1);
+      const double t_s = xs - (double)ci;
+      double t_t;
+      const int cj = periodic_cell(ts_l, P.nth_scale, P.nth, t_t);
+      const int lr = ci - row_base;
+      int lc = cj - cellcol_base;
+      if (lc >= P.nth) lc -= P.nth;
+      if (lc < 0) lc += P.nth;
+      if (mt.n < 256 && lr >= 0 && lr < kCH && lc >= 0 && lc < kCW) {
+        const unsigned int cell = (unsigned)(lr * kCW + lc);
+        S.rec[q] = make_double2(t_s, t_t);
+        const unsigned int rank = atomicAdd(&S.count[cell], 1u);
+        S.meta[q] = (ms << 21) | (rank << 9) | cell;
+      } else {
+        // footprint leaves the tile (long ring, or phi rounding): global atomics
+        S.meta[q] = (ms << 21) | kNoCell;
+        ++my_fallback;
+        const double* e = S.mtab + (size_t)ms * 5;
+        deposit_point_global<G>(P, s_l, ts_l, mt.k0, e, e[4], rho, jpar);
+      }
+    }
+    __syncthreads();
+    ORB_CLK(2);   // phase 1b
+
+    // ------------------------------------------------------------------ phase 1c: sort by cell
     if (wid == 0) {
-      // exclusive scan of the kCells counts: 15 consecutive cells per lane
+      // exclusive scan of the kCells counts, each padded to a multiple of 4: 9 cells per lane
       constexpr int per = (kCells + 31) / 32;
       unsigned int loc[per];
       unsigned int sum = 0;
 #pragma unroll
       for (int x = 0; x < per; ++x) {
         const int c = lane * per + x;
-        loc[x] = c < kCells ? S.count[c] : 0;
+        loc[x] = c < kCells ? ((S.count[c] + 3u) & ~3u) : 0;
         sum += loc[x];
       }
       unsigned int inc = sum;
@@ -351,107 +388,167 @@ k_deposit_tile(const Params P, const Markers M, const uint32_t* __restrict__ cel
 #pragma unroll
       for (int x = 0; x < per; ++x) {
         const int c = lane * per + x;
-        if (c < kCells) {
-          S.cstart[c] = ex;
-          S.count[c] = ex;   // running cursor for the permutation
-        }
+        if (c < kCells) S.cstart[c] = ex;
         ex += loc[x];
       }
       if (lane == 31) S.cstart[kCells] = inc;
+    } else {
+      // mtmp is dead from here on: its storage becomes perm, pre-filled with the dummy point
+      const unsigned int fill = (unsigned)kPCap | ((unsigned)kMCap << 16);
+      for (int x = tid - 32; x < kPermCap; x += kThreads - 32) S.perm[x] = fill;
     }
     __syncthreads();
     for (unsigned int q = tid; q < n_rec; q += kThreads) {
-      const unsigned short c = S.pcell[q];
-      if (c != kNoCell) {
-        const unsigned int pos = atomicAdd(&S.count[c], 1u);
-        S.perm[pos] = (unsigned short)q;
-      }
+      const unsigned int m = S.meta[q];
+      const unsigned int c = m & 0x1ffu;
+      if (c != kNoCell) S.perm[S.cstart[c] + ((m >> 9) & 0xfffu)] = q | ((m >> 21) << 16);
     }
     __syncthreads();
+    ORB_CLK(3);   // phase 1c
 
-    // ------------------------------------------------------------------ phase 2
+    // ------------------------------------------------------------------ phase 2: contraction
     {
-      const int g = lane >> 2, kk = lane & 3;
-      // lane's spline piece: g < 4 -> radial basis g of the current row's cell (coefficients
-      // loaded per row); g >= 4 -> cardinal theta* piece g - 4
+      const int g = lane >> 2, kk = lane & 3, hi = lane >> 4, a = g & 3;
+      // lane's spline piece: lanes 0-15 -> radial basis a of the row's cell (coefficients loaded
+      // per row) at t_s; lanes 16-31 -> cardinal theta* piece a at t_theta
       double k0c, k1c, k2c, k3c;
-      {
-        const int b = g & 3;
-        k0c = (b == 0 || b == 2) ? (1.0 / 6.0) : (b == 1 ? (2.0 / 3.0) : 0.0);
-        k1c = (b == 0) ? -0.5 : (b == 2 ? 0.5 : 0.0);
-        k2c = (b == 0 || b == 2) ? 0.5 : (b == 1 ? -1.0 : 0.0);
-        k3c = (b == 0) ? (-1.0 / 6.0) : (b == 1 ? 0.5 : (b == 2 ? -0.5 : (1.0 / 6.0)));
-      }
-      const int src_ws0 = 4 * (g >> 2) + kk;         // lane holding ws[a = g>>2] of point kk
-      const int src_ws1 = 4 * (2 + (g >> 2)) + kk;   // ws[a = 2 + (g>>2)]
-      const int src_wt = 4 * (4 + (g & 3)) + kk;     // wt[b = g&3]
+      k0c = (a == 0 || a == 2) ? (1.0 / 6.0) : (a == 1 ? (2.0 / 3.0) : 0.0);
+      k1c = (a == 0) ? -0.5 : (a == 2 ? 0.5 : 0.0);
+      k2c = (a == 0 || a == 2) ? 0.5 : (a == 1 ? -1.0 : 0.0);
+      k3c = (a == 0) ? (-1.0 / 6.0) : (a == 1 ? 0.5 : (a == 2 ? -0.5 : (1.0 / 6.0)));
+      const int src_ws = 4 * a + kk;   // lane holding ws[a] of point kk
+      int src_wt[4];                   // phase u: lane holding wt[(slot - u) & 3], slot = hi (+2)
+#pragma unroll
+      for (int u = 0; u < 4; ++u) src_wt[u] = 4 * (4 + ((hi - u) & 3)) + kk;
+      const double* recd = reinterpret_cast<const double*>(S.rec) + hi;
+      const double* mt_a = S.mtab + a;
+
       for (;;) {
         int item = 0;
         if (lane == 0) item = atomicAdd(&S.next_item, 1);
         item = __shfl_sync(kFull, item, 0);
         if (item >= kItems) break;
-        const int lr = item / kSegs, sg = item - lr * kSegs;
+#ifdef ORB_PHASE_CLOCKS
+        if (tid == 0) atomicAdd(d_points + 9, 1ull);
+#endif
+        // heavy items (rows owned by the tile) first, halo rows last
+        int lr, sg = item & 1;
+        if (item < kTileI * kSegs) {
+          lr = kHaloS + (item >> 1);
+        } else {
+          const int h = (item - kTileI * kSegs) >> 1;
+          lr = (h < kHaloS) ? h : kTileI + h;
+        }
         const int c_first = lr * kCW + sg * kSegW;
-        if (S.cstart[c_first + kSegW] == S.cstart[c_first]) continue;   // no point in the segment
+        double* pbase = S.partial + (size_t)(lr * kSegs + sg) * (kSegN * 32) + a * 8 + 2 * kk;
+        if (S.cstart[c_first + kSegW] == S.cstart[c_first]) {   // no point in the segment
+          if (chunk == 0) {
+            double2* z = reinterpret_cast<double2*>(S.partial + (size_t)(lr * kSegs + sg) * (kSegN * 32));
+            for (int x = lane; x < kSegN * 16; x += 32) z[x] = make_double2(0.0, 0.0);
+          }
+          continue;
+        }
         const int irow = row_base + lr;   // radial cell; points exist only where 0 <= irow < ns
         double q0 = k0c, q1 = k1c, q2 = k2c, q3 = k3c;
-        if (g < 4) {
-          const double* tb = P.scoef + ((size_t)irow * 4 + g) * 4;
+        if (!hi) {
+          const double* tb = P.scoef + ((size_t)irow * 4 + a) * 4;
           q0 = __ldg(tb); q1 = __ldg(tb + 1); q2 = __ldg(tb + 2); q3 = __ldg(tb + 3);
         }
-        double c00 = 0.0, c01 = 0.0, c10 = 0.0, c11 = 0.0;
-        int live = 0;   // node columns of the accumulators that may be non-zero
-        for (int step = 0; step < kSegW + 3; ++step) {
-          const int lc = sg * kSegW + step;
-          if (step < kSegW) {
-            const int cell = c_first + step;
-            const unsigned int start = S.cstart[cell];
-            const int cnt = (int)(S.cstart[cell + 1] - start);
-            if (cnt > 0) live = 4;
-            for (int p0 = 0; p0 < cnt; p0 += 4) {
-              const bool valid = p0 + kk < cnt;
-              const unsigned int qi = valid ? S.perm[start + p0 + kk] : S.perm[start];
-              const double2 t = S.rec[qi];
-              const unsigned int mk = S.pmark[qi];
-              const double tt = (g < 4) ? t.x : t.y;
+        double c0a = 0.0, c0b = 0.0, c1a = 0.0, c1b = 0.0;
+        double e0a = 0.0, e0b = 0.0, e1a = 0.0, e1b = 0.0;
+
+#define ORB_RETIRE(U, NCOL)                                                          \
+        {                                                                            \
+          double2* dst = reinterpret_cast<double2*>(pbase + (NCOL) * 32);            \
+          if ((U) < 2) {                                                             \
+            if (hi == (U)) {                                                         \
+              double2 v = make_double2(c0a + e0a, c0b + e0b);                        \
+              if (chunk) { const double2 o = *dst; v.x += o.x; v.y += o.y; }         \
+              *dst = v;                                                              \
+              c0a = 0.0; c0b = 0.0; e0a = 0.0; e0b = 0.0;                            \
+            }                                                                        \
+          } else {                                                                   \
+            if (hi == (U) - 2) {                                                     \
+              double2 v = make_double2(c1a + e1a, c1b + e1b);                        \
+              if (chunk) { const double2 o = *dst; v.x += o.x; v.y += o.y; }         \
+              *dst = v;                                                              \
+              c1a = 0.0; c1b = 0.0; e1a = 0.0; e1b = 0.0;                            \
+            }                                                                        \
+          }                                                                          \
+        }
+
+        for (int cc = 0; cc < kSegW; cc += 4) {
+#pragma unroll
+          for (int u = 0; u < 4; ++u) {
+            const int cell = c_first + cc + u;
+            const unsigned int end = S.cstart[cell + 1];
+            unsigned int pos = S.cstart[cell] + kk;
+            // two batches of 4 points per trip on independent accumulators (the loop is one
+            // warp's serial chain: without this it issues one instruction per ~8 clocks)
+            for (; pos + 4 < end; pos += 8) {
+              const unsigned int pe = S.perm[pos], pf = S.perm[pos + 4];
+              const unsigned int qi = pe & 0xffffu, mk = pe >> 16;
+              const unsigned int qj = pf & 0xffffu, ml = pf >> 16;
+              const double tt = recd[2 * qi], tu = recd[2 * qj];
+              double b = mt_a[mk * 5], bb = mt_a[ml * 5];
+              if (G == 2) {
+                const double vp = S.mtab[mk * 5 + 4], vq = S.mtab[ml * 5 + 4];
+                if (hi) { b *= vp; bb *= vq; }
+              } else {
+                if (hi) { b = 0.0; bb = 0.0; }
+              }
               const double val = fma(fma(fma(q3, tt, q2), tt, q1), tt, q0);
-              const double ws0 = __shfl_sync(kFull, val, src_ws0);
-              const double ws1 = __shfl_sync(kFull, val, src_ws1);
-              const double wt = __shfl_sync(kFull, val, src_wt);
-              double b = S.mtab[mk * 5 + (g & 3)];
-              if (G == 2 && g >= 4) b *= S.mtab[mk * 5 + 4];
-              if (!valid || (G == 1 && g >= 4)) b = 0.0;
-              dmma884(c00, c01, ws0 * wt, b);
-              dmma884(c10, c11, ws1 * wt, b);
+              const double vbl = fma(fma(fma(q3, tu, q2), tu, q1), tu, q0);
+              const double ws = __shfl_sync(kFull, val, src_ws);
+              const double xs = __shfl_sync(kFull, vbl, src_ws);
+              const double wt1 = __shfl_sync(kFull, val, src_wt[u]);
+              const double xt1 = __shfl_sync(kFull, vbl, src_wt[u]);
+              const double wt2 = __shfl_sync(kFull, val, src_wt[(u + 2) & 3]);
+              const double xt2 = __shfl_sync(kFull, vbl, src_wt[(u + 2) & 3]);
+              dmma884(c0a, c0b, ws * wt1, b);
+              dmma884(e0a, e0b, xs * xt1, bb);
+              dmma884(c1a, c1b, ws * wt2, b);
+              dmma884(e1a, e1b, xs * xt2, bb);
             }
-          }
-          if (live > 0) {
-            // retire node column lc (b = 0): nodes (lr + a, lc), a = 2m + (g>>2), channels 2kk, 2kk+1
-            if ((g & 3) == 0 && kk < 2 * G) {
-              double* t0 = S.tile + ((size_t)(lr + (g >> 2)) * kNW + lc) * NC + 2 * kk;
-              atomicAdd(t0, c00);
-              atomicAdd(t0 + 1, c01);
-              double* t1 = t0 + (size_t)2 * kNW * NC;
-              atomicAdd(t1, c10);
-              atomicAdd(t1 + 1, c11);
+            if (pos < end) {
+              const unsigned int pe = S.perm[pos];
+              const unsigned int qi = pe & 0xffffu, mk = pe >> 16;
+              const double tt = recd[2 * qi];
+              double b = mt_a[mk * 5];
+              if (G == 2) {
+                const double vp = S.mtab[mk * 5 + 4];
+                if (hi) b *= vp;
+              } else {
+                if (hi) b = 0.0;
+              }
+              const double val = fma(fma(fma(q3, tt, q2), tt, q1), tt, q0);
+              const double ws = __shfl_sync(kFull, val, src_ws);
+              const double wt1 = __shfl_sync(kFull, val, src_wt[u]);
+              const double wt2 = __shfl_sync(kFull, val, src_wt[(u + 2) & 3]);
+              dmma884(c0a, c0b, ws * wt1, b);
+              dmma884(c1a, c1b, ws * wt2, b);
             }
-            c00 = __shfl_down_sync(kFull, c00, 4);
-            c01 = __shfl_down_sync(kFull, c01, 4);
-            c10 = __shfl_down_sync(kFull, c10, 4);
-            c11 = __shfl_down_sync(kFull, c11, 4);
-            if ((g & 3) == 3) c00 = c01 = c10 = c11 = 0.0;
-            --live;
+            ORB_RETIRE(u, cc + u)
           }
         }
+        ORB_RETIRE(0, kSegW)
+        ORB_RETIRE(1, kSegW + 1)
+        ORB_RETIRE(2, kSegW + 2)
+#undef ORB_RETIRE
       }
     }
+#ifdef ORB_PHASE_CLOCKS
+    if (tid == 0) atomicAdd(d_points + 8, (unsigned long long)(clock64() - clk__));
+#endif
     __syncthreads();
+    ORB_CLK(4);   // phase 2
 
     // ------------------------------------------------------------------ next chunk?
     const bool more = S.n_deferred[cur ^ 1] > 0 || S.next_group < n_groups;
     __syncthreads();
     if (!more) break;
     cur ^= 1;
+    ++chunk;
     if (tid == 0) {
       S.n_deferred[cur ^ 1] = 0;
       S.take_deferred = 0;
@@ -465,28 +562,42 @@ k_deposit_tile(const Params P, const Markers M, const uint32_t* __restrict__ cel
     __syncthreads();
   }
 
-  // a9: one flush of the tile; consecutive lanes run along the 4 phi planes of a node (one
-  // 32-byte sector of the k-fastest grid)
-  int kpl[4];
+  // a9: sum the partial array into nodes and flush the tile once.  A thread owns one (node
+  // column, channel) and walks down the node rows; 8 consecutive lanes run along the channels
+  // of a node (4 phi planes = one 32-byte sector of the k-fastest grid, per grid).  The radial
+  // offset a is visited in an order rotated by the node column so that the 4 nodes a warp reads
+  // at once fall into different bank groups.
+  {
+    const int ch = tid & 7, t2 = tid >> 3;
+    const int half = t2 >= kNW ? 1 : 0;
+    const int tc = t2 - half * kNW;
+    if (t2 < 2 * kNW && (G == 2 || ch < 4)) {
+      int gj = (cellcol_base - 1 + tc) % P.nth;
+      if (gj < 0) gj += P.nth;
+      double* __restrict__ out = (ch < 4 ? rho : jpar) + (int64_t)gj * P.nph +
+                                 wrap_index(k - 1 + (ch & 3), P.nph);
+      const int64_t row_stride = (int64_t)P.nth * P.nph;
+      const int sg_lo = tc >= kSegN ? 1 : 0;              // segments whose columns include tc
+      const int sg_hi = tc >= kSegW ? 1 : 0;
+      const int nr_lo = half ? (kNH + 1) / 2 : 0, nr_hi = half ? kNH : (kNH + 1) / 2;
+      for (int nr = nr_lo; nr < nr_hi; ++nr) {
+        const int gi = row_base + nr;
+        if (gi < 0 || gi > P.ns + 2) continue;
+        double v = 0.0;
 #pragma unroll
-  for (int d = 0; d < 4; ++d) kpl[d] = wrap_index(k - 1 + d, P.nph);
-  for (int x = tid; x < kNH * kNW * 4; x += kThreads) {
-    const int d = x & 3;
-    const int node = x >> 2;
-    const int nr = node / kNW, ncol = node - nr * kNW;
-    const int gi = row_base + nr;
-    if (gi < 0 || gi > P.ns + 2) continue;
-    int gj = (cellcol_base - 1 + ncol) % P.nth;
-    if (gj < 0) gj += P.nth;
-    const int64_t idx = ((int64_t)gi * P.nth + gj) * (int64_t)P.nph + kpl[d];
-    const double vr = S.tile[(size_t)node * NC + d];
-    if (vr != 0.0) atomicAdd(rho + idx, vr);
-    if (G == 2) {
-      const double vj = S.tile[(size_t)node * NC + 4 + d];
-      if (vj != 0.0) atomicAdd(jpar + idx, vj);
+        for (int j = 0; j < 4; ++j) {
+          const int a = (j + tc) & 3;
+          const int lr = nr - a;
+          if (lr < 0 || lr >= kCH) continue;
+          for (int sg = sg_lo; sg <= sg_hi; ++sg)
+            v += S.partial[((lr * kSegs + sg) * kSegN + (tc - sg * kSegW)) * 32 + a * 8 + ch];
+        }
+        if (v != 0.0) atomicAdd(out + gi * row_stride, v);
+      }
     }
   }
 
+  ORB_CLK(5);   // flush (thread 0's share)
 #pragma unroll
   for (int o = 16; o > 0; o >>= 1) {
     my_points += __shfl_down_sync(kFull, my_points, o);
@@ -503,12 +614,12 @@ int launch(const Params& P, const Markers& M, const uint32_t* cell_start, double
            unsigned long long* d_points, cudaStream_t st) {
   const int tiles_i = (P.ns + kTileI - 1) / kTileI;
   const int tiles_j = (P.nth + kTileJ - 1) / kTileJ;
-  const int64_t blocks = (int64_t)tiles_i * tiles_j * P.nph;
+  const dim3 blocks((unsigned)tiles_j, (unsigned)tiles_i, (unsigned)P.nph);
   const size_t smem = sizeof(Smem<G>);
   if (cudaFuncSetAttribute(k_deposit_tile<G>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                            (int)smem) != cudaSuccess)
     return -1;
-  k_deposit_tile<G><<<(unsigned int)blocks, kThreads, smem, st>>>(P, M, cell_start, rho, jpar,
+  k_deposit_tile<G><<<blocks, kThreads, smem, st>>>(P, M, cell_start, rho, jpar,
                                                                    d_points, tiles_i, tiles_j);
   return 1;
 }

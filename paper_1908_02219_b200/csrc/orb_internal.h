@@ -11,6 +11,7 @@
 namespace orb {
 
 constexpr double kTwoPi = 6.283185307179586476925286766559;
+constexpr int kCounters = 16;    // device counters: [0] Larmor points, [1] direct-path points, [2..] debug
 constexpr int kRecDoubles = 6;  // binned marker record: s, theta*, phi, vpar, mu, w
 
 // Everything a kernel needs to know about grid, geometry, species and N_L policy.
