@@ -51,7 +51,8 @@ namespace orb {
 
 namespace {
 
-constexpr int kThreads = 512;
+constexpr int kThreads = 256;
+constexpr int kCtasPerSm = 3;
 constexpr int kWarps = kThreads / 32;
 constexpr int kTileI = 8;     // radial cells per tile
 constexpr int kTileJ = 16;    // poloidal cells per tile
@@ -66,9 +67,9 @@ constexpr int kSegW = 12;                  // cells per walk segment
 constexpr int kSegs = kCW / kSegW;         // 2
 constexpr int kSegN = kSegW + 3;           // node columns a segment produces (15)
 constexpr int kItems = kCH * kSegs;        // 24
-constexpr int kPCap = 3072;   // Larmor points per chunk
-constexpr int kMCap = 768;    // markers per chunk
-constexpr int kPermCap = ((kPCap + 3 * kCells + 3) / 4) * 4;   // points + padding to batches of 4
+constexpr int kPCap = 1024;   // Larmor points per chunk
+constexpr int kMCap = 256;    // markers per chunk
+constexpr int kPermCap = kPCap + 3 * kCells;   // points + padding to batches of 4
 constexpr unsigned kFull = 0xffffffffu;
 constexpr unsigned kNoCell = 0x1ffu;       // meta cell field of a point deposited directly
 static_assert(kCW % kSegW == 0 && kSegW % 4 == 0, "segments must tile the row in groups of 4");
@@ -88,9 +89,9 @@ struct MarkerTmp {      // phase 1a -> 1b hand-over, 32 bytes
 
 template <int G>
 struct Smem {
-  double partial[kItems * kSegN * 32];   // [row segment][node col][a][grid*4 + phi plane]
+  double tile[kNH * kNW * 8];            // [node row][node col][grid*4 + phi plane]
   double2 rec[kPCap + 1];                // (t_s, t_theta) of a Larmor point; [kPCap] = dummy
-  double mtab[(kMCap + 1) * 5];          // per marker: c*wphi[0..3], vpar; [kMCap] = dummy (zeros)
+  double mtab[(kMCap + 1) * 8];          // per marker: c*wphi[0..3], c*vpar*wphi[0..3]; [kMCap] = dummy (zeros)
   union {
     MarkerTmp mtmp[kMCap];               // phases 1a-1b
     unsigned int perm[kPermCap];         // phases 1c-2: points grouped by cell, each cell padded
@@ -141,7 +142,7 @@ __device__ __forceinline__ int periodic_cell(double u, double scale, int n, doub
 // Direct deposition of one Larmor point with global atomics (points outside the tile's halo).
 template <int G>
 __device__ __noinline__ void deposit_point_global(const Params& P, double s_l, double ts_l, int k0,
-                                                  const double* cw, double vpar,
+                                                  const double* cw, const double* cwv,
                                                   double* __restrict__ rho,
                                                   double* __restrict__ jpar) {
   double ws[4], wt[4];
@@ -157,14 +158,14 @@ __device__ __noinline__ void deposit_point_global(const Params& P, double s_l, d
       for (int d = 0; d < 4; ++d) {
         const int kk = wrap_index(k0 + d, P.nph);
         atomicAdd(rho + row + kk, v * cw[d]);
-        if (G == 2) atomicAdd(jpar + row + kk, v * cw[d] * vpar);
+        if (G == 2) atomicAdd(jpar + row + kk, v * cwv[d]);
       }
     }
   }
 }
 
 template <int G>   // G = 1: rho only; G = 2: rho and jpar
-__global__ void __launch_bounds__(kThreads, 1)
+__global__ void __launch_bounds__(kThreads, kCtasPerSm)
 k_deposit_tile(const Params P, const Markers M, const uint32_t* __restrict__ cell_start,
                double* __restrict__ rho, double* __restrict__ jpar,
                unsigned long long* __restrict__ d_points, int tiles_i, int tiles_j) {
@@ -207,7 +208,7 @@ k_deposit_tile(const Params P, const Markers M, const uint32_t* __restrict__ cel
     S.rec[kPCap] = make_double2(0.0, 0.0);
     S.meta[kPCap] = (unsigned)kMCap << 21;
 #pragma unroll
-    for (int d = 0; d < 5; ++d) S.mtab[kMCap * 5 + d] = 0.0;
+    for (int d = 0; d < 8; ++d) S.mtab[kMCap * 8 + d] = 0.0;
   }
   __syncthreads();
   const uint32_t n_tile = S.row_off[kTileI];
@@ -215,6 +216,7 @@ k_deposit_tile(const Params P, const Markers M, const uint32_t* __restrict__ cel
   const int n_groups = (int)((n_tile + 31) / 32);
 
   for (int x = tid; x <= kCells; x += kThreads) S.count[x] = 0;
+  for (int x = tid; x < kNH * kNW * 8; x += kThreads) S.tile[x] = 0.0;
   __syncthreads();
 
   ORB_CLK(0);   // prologue
@@ -305,8 +307,11 @@ k_deposit_tile(const Params P, const Markers M, const uint32_t* __restrict__ cel
 
       const unsigned int ms = mb + (unsigned)lane;
       {
-        double* e = S.mtab + (size_t)ms * 5;
-        e[0] = cw[0]; e[1] = cw[1]; e[2] = cw[2]; e[3] = cw[3]; e[4] = vpar;
+        double2* e = reinterpret_cast<double2*>(S.mtab + (size_t)ms * 8);
+        e[0] = make_double2(cw[0], cw[1]);
+        e[1] = make_double2(cw[2], cw[3]);
+        e[2] = make_double2(cw[0] * vpar, cw[1] * vpar);
+        e[3] = make_double2(cw[2] * vpar, cw[3] * vpar);
         MarkerTmp t;
         t.a = ga; t.b = gb; t.rho = grho;
         t.n = n | (k_ok ? 0 : 256);
@@ -359,8 +364,8 @@ k_deposit_tile(const Params P, const Markers M, const uint32_t* __restrict__ cel
         // footprint leaves the tile (long ring, or phi rounding): global atomics
         S.meta[q] = (ms << 21) | kNoCell;
         ++my_fallback;
-        const double* e = S.mtab + (size_t)ms * 5;
-        deposit_point_global<G>(P, s_l, ts_l, mt.k0, e, e[4], rho, jpar);
+        const double* e = S.mtab + (size_t)ms * 8;
+        deposit_point_global<G>(P, s_l, ts_l, mt.k0, e, e + 4, rho, jpar);
       }
     }
     __syncthreads();
@@ -409,19 +414,7 @@ k_deposit_tile(const Params P, const Markers M, const uint32_t* __restrict__ cel
     // ------------------------------------------------------------------ phase 2: contraction
     {
       const int g = lane >> 2, kk = lane & 3, hi = lane >> 4, a = g & 3;
-      // lane's spline piece: lanes 0-15 -> radial basis a of the row's cell (coefficients loaded
-      // per row) at t_s; lanes 16-31 -> cardinal theta* piece a at t_theta
-      double k0c, k1c, k2c, k3c;
-      k0c = (a == 0 || a == 2) ? (1.0 / 6.0) : (a == 1 ? (2.0 / 3.0) : 0.0);
-      k1c = (a == 0) ? -0.5 : (a == 2 ? 0.5 : 0.0);
-      k2c = (a == 0 || a == 2) ? 0.5 : (a == 1 ? -1.0 : 0.0);
-      k3c = (a == 0) ? (-1.0 / 6.0) : (a == 1 ? 0.5 : (a == 2 ? -0.5 : (1.0 / 6.0)));
-      const int src_ws = 4 * a + kk;   // lane holding ws[a] of point kk
-      int src_wt[4];                   // phase u: lane holding wt[(slot - u) & 3], slot = hi (+2)
-#pragma unroll
-      for (int u = 0; u < 4; ++u) src_wt[u] = 4 * (4 + ((hi - u) & 3)) + kk;
-      const double* recd = reinterpret_cast<const double*>(S.rec) + hi;
-      const double* mt_a = S.mtab + a;
+      const double* mt_g = S.mtab + g;
 
       for (;;) {
         int item = 0;
@@ -440,101 +433,76 @@ k_deposit_tile(const Params P, const Markers M, const uint32_t* __restrict__ cel
           lr = (h < kHaloS) ? h : kTileI + h;
         }
         const int c_first = lr * kCW + sg * kSegW;
-        double* pbase = S.partial + (size_t)(lr * kSegs + sg) * (kSegN * 32) + a * 8 + 2 * kk;
-        if (S.cstart[c_first + kSegW] == S.cstart[c_first]) {   // no point in the segment
-          if (chunk == 0) {
-            double2* z = reinterpret_cast<double2*>(S.partial + (size_t)(lr * kSegs + sg) * (kSegN * 32));
-            for (int x = lane; x < kSegN * 16; x += 32) z[x] = make_double2(0.0, 0.0);
-          }
-          continue;
-        }
-        const int irow = row_base + lr;   // radial cell; points exist only where 0 <= irow < ns
-        double q0 = k0c, q1 = k1c, q2 = k2c, q3 = k3c;
-        if (!hi) {
-          const double* tb = P.scoef + ((size_t)irow * 4 + a) * 4;
-          q0 = __ldg(tb); q1 = __ldg(tb + 1); q2 = __ldg(tb + 2); q3 = __ldg(tb + 3);
-        }
+        if (S.cstart[c_first + kSegW] == S.cstart[c_first]) continue;   // no point in the segment
+        // node (row lr + a, column sg*kSegW + n), channels 2kk, 2kk+1
+        double* pbase = S.tile + ((lr + a) * kNW + sg * kSegW) * 8 + 2 * kk;
+        int idle = 4;   // cells since the last one that had points: >= 4 means all slots are zero
+        // radial basis a of the row's cell: cubic in t_s (clamped ends differ from the cardinal one)
+        const int irow = row_base + lr;   // points exist only where 0 <= irow < ns
+        const double* tb = P.scoef + ((size_t)irow * 4 + a) * 4;
+        const double q0 = __ldg(tb), q1 = __ldg(tb + 1), q2 = __ldg(tb + 2), q3 = __ldg(tb + 3);
         double c0a = 0.0, c0b = 0.0, c1a = 0.0, c1b = 0.0;
-        double e0a = 0.0, e0b = 0.0, e1a = 0.0, e1b = 0.0;
+
+        // One batch = 4 points (lane's point: kk).  Every lane evaluates its own operands: the
+        // radial weight ws_a (3 FMA) and, from y = t or 1 - t, the two cardinal theta* pieces its
+        // slots need in phase U: A = y^3/6 and B = 2/3 - y^2 + y^3/2 cover all four pieces
+        // (w0(t) = A(1-t), w1(t) = B(t), w2(t) = B(1-t), w3(t) = A(t)).  No shuffles.
+#define ORB_BATCH(U, POS)                                                            \
+        {                                                                            \
+          const unsigned int pe = S.perm[POS];                                       \
+          const double2 t = S.rec[pe & 0xffffu];                                     \
+          const double b = mt_g[(pe >> 16) * 8];                                     \
+          const double ws = fma(fma(fma(q3, t.x, q2), t.x, q1), t.x, q0);            \
+          const int p1 = (hi - (U)) & 3;                                             \
+          const double y = (p1 & 1) ? t.y : 1.0 - t.y;                               \
+          const double y2 = y * y;                                                   \
+          const double y3 = y2 * y;                                                  \
+          const double wA = y3 * (1.0 / 6.0);                                        \
+          const double wB = fma(y3, 0.5, (2.0 / 3.0) - y2);                          \
+          const bool fa = (p1 == 0) || (p1 == 3);                                    \
+          dmma884(c0a, c0b, ws * (fa ? wA : wB), b);                                 \
+          dmma884(c1a, c1b, ws * (fa ? wB : wA), b);                                 \
+        }
 
 #define ORB_RETIRE(U, NCOL)                                                          \
-        {                                                                            \
-          double2* dst = reinterpret_cast<double2*>(pbase + (NCOL) * 32);            \
+        if (idle < 4) {                                                              \
+          double* dst = pbase + (NCOL) * 8;                                          \
           if ((U) < 2) {                                                             \
             if (hi == (U)) {                                                         \
-              double2 v = make_double2(c0a + e0a, c0b + e0b);                        \
-              if (chunk) { const double2 o = *dst; v.x += o.x; v.y += o.y; }         \
-              *dst = v;                                                              \
-              c0a = 0.0; c0b = 0.0; e0a = 0.0; e0b = 0.0;                            \
+              atomicAdd(dst, c0a);                                                   \
+              atomicAdd(dst + 1, c0b);                                               \
+              c0a = 0.0; c0b = 0.0;                                                  \
             }                                                                        \
           } else {                                                                   \
             if (hi == (U) - 2) {                                                     \
-              double2 v = make_double2(c1a + e1a, c1b + e1b);                        \
-              if (chunk) { const double2 o = *dst; v.x += o.x; v.y += o.y; }         \
-              *dst = v;                                                              \
-              c1a = 0.0; c1b = 0.0; e1a = 0.0; e1b = 0.0;                            \
+              atomicAdd(dst, c1a);                                                   \
+              atomicAdd(dst + 1, c1b);                                               \
+              c1a = 0.0; c1b = 0.0;                                                  \
             }                                                                        \
           }                                                                          \
         }
 
+#pragma unroll 1
         for (int cc = 0; cc < kSegW; cc += 4) {
 #pragma unroll
           for (int u = 0; u < 4; ++u) {
             const int cell = c_first + cc + u;
             const unsigned int end = S.cstart[cell + 1];
             unsigned int pos = S.cstart[cell] + kk;
-            // two batches of 4 points per trip on independent accumulators (the loop is one
-            // warp's serial chain: without this it issues one instruction per ~8 clocks)
-            for (; pos + 4 < end; pos += 8) {
-              const unsigned int pe = S.perm[pos], pf = S.perm[pos + 4];
-              const unsigned int qi = pe & 0xffffu, mk = pe >> 16;
-              const unsigned int qj = pf & 0xffffu, ml = pf >> 16;
-              const double tt = recd[2 * qi], tu = recd[2 * qj];
-              double b = mt_a[mk * 5], bb = mt_a[ml * 5];
-              if (G == 2) {
-                const double vp = S.mtab[mk * 5 + 4], vq = S.mtab[ml * 5 + 4];
-                if (hi) { b *= vp; bb *= vq; }
-              } else {
-                if (hi) { b = 0.0; bb = 0.0; }
-              }
-              const double val = fma(fma(fma(q3, tt, q2), tt, q1), tt, q0);
-              const double vbl = fma(fma(fma(q3, tu, q2), tu, q1), tu, q0);
-              const double ws = __shfl_sync(kFull, val, src_ws);
-              const double xs = __shfl_sync(kFull, vbl, src_ws);
-              const double wt1 = __shfl_sync(kFull, val, src_wt[u]);
-              const double xt1 = __shfl_sync(kFull, vbl, src_wt[u]);
-              const double wt2 = __shfl_sync(kFull, val, src_wt[(u + 2) & 3]);
-              const double xt2 = __shfl_sync(kFull, vbl, src_wt[(u + 2) & 3]);
-              dmma884(c0a, c0b, ws * wt1, b);
-              dmma884(e0a, e0b, xs * xt1, bb);
-              dmma884(c1a, c1b, ws * wt2, b);
-              dmma884(e1a, e1b, xs * xt2, bb);
-            }
-            if (pos < end) {
-              const unsigned int pe = S.perm[pos];
-              const unsigned int qi = pe & 0xffffu, mk = pe >> 16;
-              const double tt = recd[2 * qi];
-              double b = mt_a[mk * 5];
-              if (G == 2) {
-                const double vp = S.mtab[mk * 5 + 4];
-                if (hi) b *= vp;
-              } else {
-                if (hi) b = 0.0;
-              }
-              const double val = fma(fma(fma(q3, tt, q2), tt, q1), tt, q0);
-              const double ws = __shfl_sync(kFull, val, src_ws);
-              const double wt1 = __shfl_sync(kFull, val, src_wt[u]);
-              const double wt2 = __shfl_sync(kFull, val, src_wt[(u + 2) & 3]);
-              dmma884(c0a, c0b, ws * wt1, b);
-              dmma884(c1a, c1b, ws * wt2, b);
-            }
+            idle = (pos < end) ? 0 : idle + 1;
+#pragma unroll 2
+            for (; pos < end; pos += 4) ORB_BATCH(u, pos)
             ORB_RETIRE(u, cc + u)
           }
         }
+        ++idle;
         ORB_RETIRE(0, kSegW)
+        ++idle;
         ORB_RETIRE(1, kSegW + 1)
+        ++idle;
         ORB_RETIRE(2, kSegW + 2)
 #undef ORB_RETIRE
+#undef ORB_BATCH
       }
     }
 #ifdef ORB_PHASE_CLOCKS
@@ -562,37 +530,22 @@ k_deposit_tile(const Params P, const Markers M, const uint32_t* __restrict__ cel
     __syncthreads();
   }
 
-  // a9: sum the partial array into nodes and flush the tile once.  A thread owns one (node
-  // column, channel) and walks down the node rows; 8 consecutive lanes run along the channels
-  // of a node (4 phi planes = one 32-byte sector of the k-fastest grid, per grid).  The radial
-  // offset a is visited in an order rotated by the node column so that the 4 nodes a warp reads
-  // at once fall into different bank groups.
+  // a9: flush the tile once.  8 consecutive lanes run along the channels of a node (4 phi planes
+  // = one 32-byte sector of the k-fastest grid, per grid).
   {
-    const int ch = tid & 7, t2 = tid >> 3;
-    const int half = t2 >= kNW ? 1 : 0;
-    const int tc = t2 - half * kNW;
-    if (t2 < 2 * kNW && (G == 2 || ch < 4)) {
-      int gj = (cellcol_base - 1 + tc) % P.nth;
-      if (gj < 0) gj += P.nth;
-      double* __restrict__ out = (ch < 4 ? rho : jpar) + (int64_t)gj * P.nph +
-                                 wrap_index(k - 1 + (ch & 3), P.nph);
-      const int64_t row_stride = (int64_t)P.nth * P.nph;
-      const int sg_lo = tc >= kSegN ? 1 : 0;              // segments whose columns include tc
-      const int sg_hi = tc >= kSegW ? 1 : 0;
-      const int nr_lo = half ? (kNH + 1) / 2 : 0, nr_hi = half ? kNH : (kNH + 1) / 2;
-      for (int nr = nr_lo; nr < nr_hi; ++nr) {
-        const int gi = row_base + nr;
-        if (gi < 0 || gi > P.ns + 2) continue;
-        double v = 0.0;
-#pragma unroll
-        for (int j = 0; j < 4; ++j) {
-          const int a = (j + tc) & 3;
-          const int lr = nr - a;
-          if (lr < 0 || lr >= kCH) continue;
-          for (int sg = sg_lo; sg <= sg_hi; ++sg)
-            v += S.partial[((lr * kSegs + sg) * kSegN + (tc - sg * kSegW)) * 32 + a * 8 + ch];
-        }
-        if (v != 0.0) atomicAdd(out + gi * row_stride, v);
+    const int ch = tid & 7;
+    double* __restrict__ out = (ch < 4 ? rho : jpar) + wrap_index(k - 1 + (ch & 3), P.nph);
+    const int64_t row_stride = (int64_t)P.nth * P.nph;
+    if (G == 2 || ch < 4) {
+      for (int node = tid >> 3; node < kNH * kNW; node += kThreads / 8) {
+        const double v = S.tile[node * 8 + ch];
+        if (v == 0.0) continue;
+        const int nr = node / kNW, tc = node - nr * kNW;
+        const int gi = row_base + nr;           // zero outside [0, ns + 2]: no point maps there
+        int gj = cellcol_base - 1 + tc;
+        while (gj < 0) gj += P.nth;
+        while (gj >= P.nth) gj -= P.nth;
+        atomicAdd(out + gi * row_stride + (int64_t)gj * P.nph, v);
       }
     }
   }
