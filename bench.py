@@ -42,10 +42,15 @@ UNIT = "Larmor points/s"
 HBM_FALLBACK_GBS = 6650.0      # /opt/skills/guides/B200_PROFILING.md fallback
 HBM_NOMINAL_GBS = 8000.0       # the "~8 TB/s" north_star quotes
 L2_BYTES = 126 << 20
+# fp64 roof of the scatter arithmetic: measured DFMA/DMMA rate of this pool's
+# B200 (profiles/r01_microbench.md: 17.9 TFMA/s = 61.7 of 64 lanes/clk/SM at 1965 MHz); nominal
+# 148 SM x 64 lanes x 2 flop x 1.965 GHz = 37.2 TFLOP/s.
+FP64_MEASURED_TFLOPS = 35.8
+FP64_NOMINAL_TFLOPS = 37.2
 
 # dram__bytes_read.sum + dram__bytes_write.sum of ONE launch of the deposit kernel, from the
 # `ncu --set full` capture summarised in profiles/ (None until a capture of that workload exists)
-NCU_TRAFFIC_BYTES = {}
+NCU_TRAFFIC_BYTES = {"cfg3": 3829880000 + 797996032}   # profiles/r01_v4_deposit_ncu.md
 
 
 def measured_hbm_peak():
@@ -305,6 +310,7 @@ def run_ours(args):
         peak, peak_src = measured_hbm_peak()
         alg_bytes = cfg.algorithmic_bytes
         achieved = alg_bytes / (dep_ms * 1e-3) / 1e9
+        flops = 2.0 * 64.0 * (2 if cfg.current else 1) * npts_step
         line = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K,
             "warmup": args.warmup, "ms_per_step": job_ms / K, "higher_is_better": True,
@@ -324,6 +330,15 @@ def run_ours(args):
                          "traffic": NCU_TRAFFIC_BYTES.get(cfg.name), "peak_source": peak_src,
                          "algorithmic_bytes": alg_bytes, "kernel_ms": dep_ms,
                          "frac_of_nominal_8TBs": achieved / HBM_NOMINAL_GBS},
+            "roofline_alu": {"bound": "alu", "pipe": "fp64", "kernel": "k_deposit_tile",
+                             "achieved": flops / (dep_ms * 1e-3) / 1e12, "peak": FP64_MEASURED_TFLOPS,
+                             "unit": "TFLOP/s",
+                             "frac": flops / (dep_ms * 1e-3) / 1e12 / FP64_MEASURED_TFLOPS,
+                             "frac_of_nominal": flops / (dep_ms * 1e-3) / 1e12 / FP64_NOMINAL_TFLOPS,
+                             "algorithmic_flops": flops,
+                             "note": "scatter only: 64 nodes x n_grids FMA per Larmor point; the "
+                                     "geometry (sincos, sqrt, atan2) is not counted; peak = measured "
+                                     "DFMA rate (profiles/r01_microbench.md)"},
             "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": up,
                     "d2h_bytes_per_step": down, "steps": E, "ms_per_step": e2e_job_ms / E,
                     "api": "orb_deposit_host (pinned host SoA in, host grids out)",

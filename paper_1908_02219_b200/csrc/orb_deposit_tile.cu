@@ -1,14 +1,16 @@
-// Tile deposition, v3 (hot-path steps a1-a6, a8, a9): register accumulation through the fp64
-// MMA unit; no atomics of any kind on the per-point path.
+// Tile deposition, v4 (hot-path steps a1-a6, a8, a9): register accumulation through the fp64
+// MMA unit, several small thread blocks per SM so that the phases of different tiles overlap.
 //
 // One thread block per grid tile = (1 toroidal cell slab k) x (kTileI radial cells) x (kTileJ
 // poloidal cells); its markers are found through the binning pass's per-cell offsets
 // (orb_bin.cu; key phi-major, so every radial row of the tile is one contiguous run).  The tile's
-// markers are processed in chunks of <= kPCap Larmor points (a cfg3 tile is one chunk); per chunk
+// markers are processed in chunks of <= kPCap Larmor points, in bin order (a chunk is a few cell
+// rows of markers, so its points fall on a compact window of cells); per chunk
 //
-//   phase 1a (one lane per marker): marker -> guiding-centre geometry, N_L, c = q w / N_L,
-//            c * phi-weights, v_par into a shared-memory marker table; a prefix sum of N_L over
-//            the warp's 32 markers allocates the slots of their Larmor points.
+//   phase 1a (one lane per marker): marker -> guiding-centre geometry, N_L, c = q w / N_L, then
+//            c * phi-weights and c * v_par * phi-weights (the 8 channel values of the marker)
+//            into a shared-memory marker table; a prefix sum of N_L over the warp's 32 markers
+//            allocates the slots of their Larmor points.
 //   phase 1b (one lane per Larmor point, all threads, evenly -- adaptive N_L = 4..32 keeps every
 //            lane busy): point -> (s_l, theta*_l) -> (s, theta*) cell + in-cell coordinates
 //            (t_s, t_theta), a 16-byte record; a per-cell counter is bumped (native 32-bit shared
@@ -22,37 +24,36 @@
 //            is the dense contraction
 //                 C[node(a,b)][channel(d,grid)] = sum_pts  ws_a(pt) wt_b(pt) * cw_d(pt) {1, vpar(pt)}
 //            = A (16 x npts) . B (npts x 8), issued as two DMMA m8n8k4 per 4 points with the
-//            accumulators in registers.  Each lane prepares ONE spline value per batch (a cubic in
-//            t with lane-constant coefficients, 3 FMA); operands are exchanged by shuffles.  The
-//            four node columns of the accumulator window live in four fixed "slots" (half-warp x
-//            DMMA); stepping to the next cell retires the slot of the finished column with one
-//            128-bit store per lane of a half-warp and re-uses it for the new column -- no data
-//            moves, only the shuffle source lanes rotate (the walk is unrolled by 4).
-//            Retired columns go to partial[row segment][node column][a][channel]: the radial
-//            offset a is kept apart, so every entry has exactly one writer and is written once
-//            per chunk -- plain stores, no read-modify-write, no atomics.
+//            accumulators in registers.  Every lane evaluates its own A operands from (t_s,
+//            t_theta) -- one radial cubic and the two cardinal theta* pieces of its slots, which
+//            are y^3/6 and 2/3 - y^2 + y^3/2 at y = t or 1 - t -- so no operand crosses lanes (the
+//            shuffle unit shares the 128 B/clk/SM load-store path, which is as scarce here as the
+//            fp64 pipe).  The four node columns of the accumulator window live in four fixed
+//            "slots" (half-warp x DMMA); stepping to the next cell retires the slot of the
+//            finished column into the shared tile (fp64 CAS add, 2 per lane of a half-warp) and
+//            re-uses it for the new column -- no data moves, only the piece a lane evaluates
+//            rotates (the walk is unrolled by 4).
 //
-// and at the end the tile's nodes are summed from the partial array (4 radial offsets, 2
-// overlapping segments) and flushed ONCE with fp64 RED.ADD to global memory.  Points whose cell
+// and at the end the tile is flushed ONCE with fp64 RED.ADD to global memory.  Points whose cell
 // leaves the tile's halo (long rings, rounding at a slab boundary) are deposited directly with
 // global atomics (rare; counted).
 //
-// Why this shape: profiles/r01_microbench.md -- shared-memory fp64 atomics are CAS loops
-// (1.5 updates/clk/SM at this access pattern) and global fp64 REDs issue at 0.78 lanes/clk/SM,
-// while the path needs 128 node updates per Larmor point; only register accumulators keep up with
-// the fp64 pipe (64 FMA/clk/SM).  DMMA runs on that same pipe at the same FMA rate (measured
-// 18.5 TFMA/s either way) but needs one operand pair per 8 FMAs, which is what makes the operand
-// traffic fit.  profiles/r01_v2_deposit_ncu.md -- v2 spent 38 warp instructions per point, 58 % of
-// them in phase 2 (window shift by shuffles, CAS retire loops); v3's slot rotation and
-// single-writer partial array remove both.
+// Why this shape (profiles/r01_microbench.md, r01_v2_deposit_ncu.md, r01_v4_deposit_ncu.md):
+// shared-memory fp64 atomics are CAS loops (1.5 updates/clk/SM) and global fp64 REDs issue at
+// 0.78 lanes/clk/SM, while the path needs 128 node updates per Larmor point; only register
+// accumulators keep up with the fp64 pipe (64 FMA/clk/SM).  DMMA m8n8k4 occupies that pipe for
+// 16 clk per SM sub-partition (same FMA rate as DFMA) but needs one operand pair per 8 FMAs.
+// One 512-thread block per SM (v2, v3) left the SM waiting at barriers and on single-warp
+// dependency chains; three 256-thread (or two 384-thread) blocks with ~70-95 KB of shared memory
+// each overlap one tile's geometry with another's contraction and flush.
 #include "orb_geom.cuh"
 
 namespace orb {
 
 namespace {
 
-constexpr int kThreads = 256;
-constexpr int kCtasPerSm = 3;
+constexpr int kThreads = 384;
+constexpr int kCtasPerSm = 2;
 constexpr int kWarps = kThreads / 32;
 constexpr int kTileI = 8;     // radial cells per tile
 constexpr int kTileJ = 16;    // poloidal cells per tile
@@ -67,8 +68,8 @@ constexpr int kSegW = 12;                  // cells per walk segment
 constexpr int kSegs = kCW / kSegW;         // 2
 constexpr int kSegN = kSegW + 3;           // node columns a segment produces (15)
 constexpr int kItems = kCH * kSegs;        // 24
-constexpr int kPCap = 1024;   // Larmor points per chunk
-constexpr int kMCap = 256;    // markers per chunk
+constexpr int kPCap = 1536;   // Larmor points per chunk
+constexpr int kMCap = 384;    // markers per chunk
 constexpr int kPermCap = kPCap + 3 * kCells;   // points + padding to batches of 4
 constexpr unsigned kFull = 0xffffffffu;
 constexpr unsigned kNoCell = 0x1ffu;       // meta cell field of a point deposited directly

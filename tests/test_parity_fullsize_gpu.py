@@ -1,0 +1,139 @@
+"""-m gpu: parity at BASELINE.json's FULL sizes, in the launch configuration bench.py times
+(bind -> orb_markers_bin -> orb_grid_zero -> orb_deposit, tile kernel).
+
+cfg1, cfg2, cfg3: the whole grid against the oracle run over all markers (marker ranges on all
+host cores, summed in fixed order -- oracle.deposit_ranges).
+cfg4 (2e8 markers, random and pre-sorted): sampled outputs the oracle can compute exactly: a
+toroidal node plane k receives contributions only from markers whose phi cell is k-2 .. k+1, so
+the oracle deposit of just those markers gives every node of that plane; three planes
+(including the periodic wrap at k = 0) are compared element by element.  Plus properties that
+hold at any size: charge/current conservation (P1) and the Larmor-point count.
+
+Tolerance (north_star, R19): max|gpu - oracle| <= 1e-12 * max|oracle| per grid.
+"""
+import os
+
+import numpy as np
+import pytest
+
+import oracle as O
+from paper_1908_02219_b200 import binding as B
+from paper_1908_02219_b200 import workloads as W
+
+from gpu_util import TOL, oracle_geom, oracle_policy, rel_err
+
+pytestmark = pytest.mark.gpu
+
+
+def _host_mem_gb():
+    try:
+        with open("/proc/meminfo") as f:
+            for line in f:
+                if line.startswith("MemAvailable"):
+                    return int(line.split()[1]) / 1e6
+    except OSError:
+        pass
+    return 0.0
+
+
+def _bench_step(cfg, d, bind_flags=0):
+    """The step bench.py times, once, on device-resident markers. -> (rho, jpar, n_points, g)"""
+    import torch
+    g = B.grid_for(cfg)
+    shape = g.shape()
+    rho = torch.full(shape, 7.0, dtype=torch.float64, device="cuda")   # must be zeroed by the step
+    jpar = torch.full(shape, -3.0, dtype=torch.float64, device="cuda") if cfg.current else None
+    st = torch.cuda.current_stream().cuda_stream
+    g.markers_bind(d["s"], d["theta"], d["phi"], d["vpar"] if cfg.current else None, d["mu"],
+                   d["w"], flags=bind_flags)
+    g.markers_bin(st)
+    g.grid_zero(rho, jpar, st)
+    g.deposit(rho, jpar, B.policy_for(cfg), st)
+    torch.cuda.synchronize()
+    npts = g.last_points()
+    fallback = g.last_fallback_points()
+    g.destroy()
+    return rho, jpar, npts, fallback
+
+
+def _conservation(cfg, m, rho, jpar):
+    scale = abs(cfg.q) * np.abs(m["w"]).sum()
+    assert abs(float(rho.sum().item()) - cfg.q * m["w"].sum()) <= 1e-11 * scale
+    if cfg.current:
+        scale_j = abs(cfg.q) * np.abs(m["w"] * m["vpar"]).sum()
+        assert abs(float(jpar.sum().item()) - cfg.q * (m["w"] * m["vpar"]).sum()) <= 1e-11 * scale_j
+
+
+@pytest.mark.parametrize("name", ["cfg1", "cfg2", "cfg3"])
+def test_full_grid_against_oracle(name):
+    import torch
+    cfg = W.CONFIGS[name]
+    m = W.generate(cfg)
+    d = {f: torch.from_numpy(m[f]).cuda() for f in W.FIELDS}
+    rho, jpar, npts, fallback = _bench_step(cfg, d)
+    del d
+    rho_o, jpar_o, npts_o, _ = O.deposit_ranges(oracle_geom(cfg), oracle_policy(cfg),
+                                                *(m[f] for f in W.FIELDS), current=cfg.current)
+    assert npts == npts_o
+    assert fallback < 0.01 * npts          # the shared-memory tile path carries the load
+    err = rel_err(rho.cpu().numpy(), rho_o)
+    assert err <= TOL, "%s rho: %.3e" % (name, err)
+    if cfg.current:
+        errj = rel_err(jpar.cpu().numpy(), jpar_o)
+        assert errj <= TOL, "%s jpar: %.3e" % (name, errj)
+    _conservation(cfg, m, rho, jpar)
+
+
+@pytest.fixture(scope="module")
+def cfg4_case():
+    if _host_mem_gb() < 60.0:
+        pytest.skip("cfg4 needs ~40 GB of host memory")
+    import torch
+    if torch.cuda.mem_get_info()[1] < 60e9:
+        pytest.skip("cfg4 needs ~25 GB of device memory")
+    cfg = W.CONFIGS["cfg4"]
+    m = W.generate(cfg)
+    og, op = oracle_geom(cfg), oracle_policy(cfg)
+    kcell = np.minimum((m["phi"] * (cfg.nphi / W.TWO_PI)).astype(np.int64), cfg.nphi - 1)
+    planes = {}
+    for k0 in (0, 37, cfg.nphi - 1):
+        near = ((kcell - k0 + 2) % cfg.nphi) < 4          # phi cells k0-2 .. k0+1
+        sub = [np.ascontiguousarray(m[f][near]) for f in W.FIELDS]
+        rho_o, jpar_o, _, _ = O.deposit_ranges(og, op, *sub, current=True)
+        planes[k0] = (rho_o[:, :, k0].copy(), jpar_o[:, :, k0].copy())
+    _, npts = O.nl_histogram(og, op, m["s"], m["theta"], m["mu"])
+    return cfg, m, planes, npts
+
+
+def _check_planes(rho, jpar, planes):
+    for k0, (rho_o, jpar_o) in planes.items():
+        got = rho[:, :, k0].cpu().numpy()
+        assert np.abs(got - rho_o).max() <= TOL * np.abs(rho_o).max(), "rho plane %d" % k0
+        gotj = jpar[:, :, k0].cpu().numpy()
+        assert np.abs(gotj - jpar_o).max() <= TOL * np.abs(jpar_o).max(), "jpar plane %d" % k0
+
+
+def test_cfg4_random_order_sampled_planes(cfg4_case):
+    import torch
+    cfg, m, planes, npts_o = cfg4_case
+    d = {f: torch.from_numpy(m[f]).cuda() for f in W.FIELDS}
+    rho, jpar, npts, fallback = _bench_step(cfg, d)
+    del d
+    assert npts == npts_o
+    assert fallback < 0.01 * npts
+    _check_planes(rho, jpar, planes)
+    _conservation(cfg, m, rho, jpar)
+
+
+def test_cfg4_presorted_sampled_planes(cfg4_case):
+    """R17: same markers pre-sorted by cell key on the host, bound with ORB_MARKERS_SORTED."""
+    import torch
+    cfg, m, planes, npts_o = cfg4_case
+    perm = np.argsort(W.cell_key(cfg, m["s"], m["theta"], m["phi"]), kind="stable")
+    d = {f: torch.from_numpy(m[f][perm]).cuda() for f in W.FIELDS}
+    del perm
+    rho, jpar, npts, fallback = _bench_step(cfg, d, bind_flags=B.ORB_MARKERS_SORTED)
+    del d
+    assert npts == npts_o
+    _check_planes(rho, jpar, planes)
+    _conservation(cfg, m, rho, jpar)
