@@ -12,7 +12,10 @@ namespace orb {
 
 constexpr double kTwoPi = 6.283185307179586476925286766559;
 constexpr int kCounters = 16;    // device counters: [0] Larmor points, [1] direct-path points, [2..] debug
-constexpr int kRecDoubles = 6;  // binned marker record: s, theta*, phi, vpar, mu, w
+// binned marker record: s, theta*, phi, vpar, mu, w + 2 doubles of padding.  64 bytes = two whole
+// 32-byte sectors, so the random-order scatter of the counting sort never leaves a partially
+// written sector for DRAM to read back (48-byte records cost 6.6 GB of fill reads on cfg3).
+constexpr int kRecDoubles = 8;
 
 // Everything a kernel needs to know about grid, geometry, species and N_L policy.
 // Passed by value as a kernel parameter.
