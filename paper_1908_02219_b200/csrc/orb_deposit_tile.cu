@@ -76,6 +76,7 @@ constexpr unsigned kNoCell = 0x1ffu;       // meta cell field of a point deposit
 static_assert(kCW % kSegW == 0 && kSegW % 4 == 0, "segments must tile the row in groups of 4");
 static_assert(kPCap >= 32 * ORB_MAX_NL && kPCap < 4096 && kMCap % 32 == 0 && kMCap < 2047, "caps");
 static_assert(kCells < (int)kNoCell, "cell id must fit 9 bits");
+static_assert(kPCap * 16 < 65536 && kMCap * 64 < 65536, "perm entries hold 16-bit byte offsets");
 
 // meta word of a point slot.  After phase 1a: marker slot << 21 | point index in the ring.
 // After phase 1b: marker slot << 21 | rank inside the cell << 9 | tile-local cell.
@@ -127,6 +128,28 @@ __device__ __forceinline__ void dmma884(double& c0, double& c1, double a, double
   asm("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};"
                : "+d"(c0), "+d"(c1)
                : "d"(a), "d"(b));
+}
+
+// dst[0] += a, dst[1] += b on a 16-byte aligned shared-memory pair, as ONE 128-bit CAS loop
+// (there is no native fp64 add on shared memory; two 64-bit CAS loops cost twice the instructions).
+__device__ __forceinline__ void smem_add2(double* dst, double a, double b) {
+  const unsigned addr = (unsigned)__cvta_generic_to_shared(dst);
+  unsigned long long c0, c1;
+  asm volatile("ld.shared.v2.b64 {%0,%1}, [%2];" : "=l"(c0), "=l"(c1) : "r"(addr));
+  for (;;) {
+    const unsigned long long n0 = __double_as_longlong(__longlong_as_double(c0) + a);
+    const unsigned long long n1 = __double_as_longlong(__longlong_as_double(c1) + b);
+    unsigned long long o0, o1;
+    asm volatile(
+        "{\n .reg .b128 c, n, o;\n mov.b128 c, {%2,%3};\n mov.b128 n, {%4,%5};\n"
+        " atom.shared.cas.b128 o, [%6], c, n;\n mov.b128 {%0,%1}, o;\n}"
+        : "=l"(o0), "=l"(o1)
+        : "l"(c0), "l"(c1), "l"(n0), "l"(n1), "r"(addr)
+        : "memory");
+    if (o0 == c0 && o1 == c1) break;
+    c0 = o0;
+    c1 = o1;
+  }
 }
 
 // angle u in [-2pi, 4pi] -> cell in [0, n) and in-cell coordinate
@@ -330,22 +353,23 @@ k_deposit_tile(const Params P, const Markers M, const uint32_t* __restrict__ cel
 
     // ------------------------------------------------------------------ phase 1b: Larmor points
     const unsigned int n_rec = min(S.npts, S.pts_end);
+    bool any_direct = false;
+#pragma unroll 2
     for (unsigned int q = tid; q < n_rec; q += kThreads) {
       const unsigned int m0 = S.meta[q];
       const unsigned int ms = meta_marker(m0);
       const int l = (int)(m0 & 0x1fu);
       const MarkerTmp mt = S.mtmp[ms];
-      double s_l, ts_l;
       const int n = mt.n & 255;
-      if (n == 1) {
+      GuidingCentre g;
+      g.x0 = mt.a;
+      g.z0 = mt.b;
+      g.rho = mt.rho;
+      double s_l, ts_l;
+      larmor_point(P, g, ring_entry(P, n, l), s_l, ts_l);
+      if (n == 1) {   // R8: the guiding centre itself, (s, theta*) as stored
         s_l = mt.a;
         ts_l = mt.b;
-      } else {
-        GuidingCentre g;
-        g.x0 = mt.a;
-        g.z0 = mt.b;
-        g.rho = mt.rho;
-        larmor_point(P, g, ring_entry(P, n, l), s_l, ts_l);
       }
       const double xs = s_l * (double)P.ns;
       const int ci = min((int)xs, P.ns - 1);
@@ -362,11 +386,21 @@ k_deposit_tile(const Params P, const Markers M, const uint32_t* __restrict__ cel
         const unsigned int rank = atomicAdd(&S.count[cell], 1u);
         S.meta[q] = (ms << 21) | (rank << 9) | cell;
       } else {
-        // footprint leaves the tile (long ring, or phi rounding): global atomics
+        // footprint leaves the tile (long ring, or phi rounding): direct path below
+        S.rec[q] = make_double2(s_l, ts_l);
         S.meta[q] = (ms << 21) | kNoCell;
-        ++my_fallback;
+        any_direct = true;
+      }
+    }
+    if (any_direct) {   // rare: global atomics for the points marked above (own slots only)
+      for (unsigned int q = tid; q < n_rec; q += kThreads) {
+        const unsigned int m0 = S.meta[q];
+        if ((m0 & 0x1ffu) != kNoCell) continue;
+        const unsigned int ms = meta_marker(m0);
+        const double2 pt = S.rec[q];
         const double* e = S.mtab + (size_t)ms * 8;
-        deposit_point_global<G>(P, s_l, ts_l, mt.k0, e, e + 4, rho, jpar);
+        ++my_fallback;
+        deposit_point_global<G>(P, pt.x, pt.y, S.mtmp[ms].k0, e, e + 4, rho, jpar);
       }
     }
     __syncthreads();
@@ -400,14 +434,14 @@ k_deposit_tile(const Params P, const Markers M, const uint32_t* __restrict__ cel
       if (lane == 31) S.cstart[kCells] = inc;
     } else {
       // mtmp is dead from here on: its storage becomes perm, pre-filled with the dummy point
-      const unsigned int fill = (unsigned)kPCap | ((unsigned)kMCap << 16);
+      const unsigned int fill = ((unsigned)kPCap * 16u) | (((unsigned)kMCap * 64u) << 16);
       for (int x = tid - 32; x < kPermCap; x += kThreads - 32) S.perm[x] = fill;
     }
     __syncthreads();
     for (unsigned int q = tid; q < n_rec; q += kThreads) {
       const unsigned int m = S.meta[q];
       const unsigned int c = m & 0x1ffu;
-      if (c != kNoCell) S.perm[S.cstart[c] + ((m >> 9) & 0xfffu)] = q | ((m >> 21) << 16);
+      if (c != kNoCell) S.perm[S.cstart[c] + ((m >> 9) & 0xfffu)] = (q * 16u) | (((m >> 21) * 64u) << 16);
     }
     __syncthreads();
     ORB_CLK(3);   // phase 1c
@@ -415,7 +449,9 @@ k_deposit_tile(const Params P, const Markers M, const uint32_t* __restrict__ cel
     // ------------------------------------------------------------------ phase 2: contraction
     {
       const int g = lane >> 2, kk = lane & 3, hi = lane >> 4, a = g & 3;
-      const double* mt_g = S.mtab + g;
+      // perm entries hold byte offsets: point slot * 16 | marker slot * 64 << 16
+      const char* rec_b = reinterpret_cast<const char*>(S.rec);
+      const char* mt_b = reinterpret_cast<const char*>(S.mtab + g);
 
       for (;;) {
         int item = 0;
@@ -451,8 +487,8 @@ k_deposit_tile(const Params P, const Markers M, const uint32_t* __restrict__ cel
 #define ORB_BATCH(U, POS)                                                            \
         {                                                                            \
           const unsigned int pe = S.perm[POS];                                       \
-          const double2 t = S.rec[pe & 0xffffu];                                     \
-          const double b = mt_g[(pe >> 16) * 8];                                     \
+          const double2 t = *reinterpret_cast<const double2*>(rec_b + (pe & 0xffffu)); \
+          const double b = *reinterpret_cast<const double*>(mt_b + (pe >> 16));      \
           const double ws = fma(fma(fma(q3, t.x, q2), t.x, q1), t.x, q0);            \
           const int p1 = (hi - (U)) & 3;                                             \
           const double y = (p1 & 1) ? t.y : 1.0 - t.y;                               \
@@ -485,6 +521,10 @@ k_deposit_tile(const Params P, const Markers M, const uint32_t* __restrict__ cel
 
 #pragma unroll 1
         for (int cc = 0; cc < kSegW; cc += 4) {
+          if (idle >= 4 && S.cstart[c_first + cc + 4] == S.cstart[c_first + cc]) {
+            idle += 4;   // four empty cells and an empty window: nothing to add or retire
+            continue;
+          }
 #pragma unroll
           for (int u = 0; u < 4; ++u) {
             const int cell = c_first + cc + u;
