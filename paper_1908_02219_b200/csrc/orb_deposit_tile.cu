@@ -109,6 +109,8 @@ struct Smem {
   unsigned int npts, nmark, pts_end;
   int full;
   int next_item;
+  int n_items;                           // row segments of this chunk that hold points
+  unsigned char item_order[kItems];      // ... heaviest first
 };
 
 #ifdef ORB_PHASE_CLOCKS
@@ -128,28 +130,6 @@ __device__ __forceinline__ void dmma884(double& c0, double& c1, double a, double
   asm("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};"
                : "+d"(c0), "+d"(c1)
                : "d"(a), "d"(b));
-}
-
-// dst[0] += a, dst[1] += b on a 16-byte aligned shared-memory pair, as ONE 128-bit CAS loop
-// (there is no native fp64 add on shared memory; two 64-bit CAS loops cost twice the instructions).
-__device__ __forceinline__ void smem_add2(double* dst, double a, double b) {
-  const unsigned addr = (unsigned)__cvta_generic_to_shared(dst);
-  unsigned long long c0, c1;
-  asm volatile("ld.shared.v2.b64 {%0,%1}, [%2];" : "=l"(c0), "=l"(c1) : "r"(addr));
-  for (;;) {
-    const unsigned long long n0 = __double_as_longlong(__longlong_as_double(c0) + a);
-    const unsigned long long n1 = __double_as_longlong(__longlong_as_double(c1) + b);
-    unsigned long long o0, o1;
-    asm volatile(
-        "{\n .reg .b128 c, n, o;\n mov.b128 c, {%2,%3};\n mov.b128 n, {%4,%5};\n"
-        " atom.shared.cas.b128 o, [%6], c, n;\n mov.b128 {%0,%1}, o;\n}"
-        : "=l"(o0), "=l"(o1)
-        : "l"(c0), "l"(c1), "l"(n0), "l"(n1), "r"(addr)
-        : "memory");
-    if (o0 == c0 && o1 == c1) break;
-    c0 = o0;
-    c1 = o1;
-  }
 }
 
 // angle u in [-2pi, 4pi] -> cell in [0, n) and in-cell coordinate
@@ -432,6 +412,23 @@ k_deposit_tile(const Params P, const Markers M, const uint32_t* __restrict__ cel
         ex += loc[x];
       }
       if (lane == 31) S.cstart[kCells] = inc;
+      __syncwarp();
+      // phase 2 work list: the row segments that hold points, heaviest first (longest processing
+      // time first keeps the warps' finishing times close: less waiting at the barrier)
+      unsigned int wgt = 0;
+      if (lane < kItems) {
+        const int c0 = (lane >> 1) * kCW + (lane & 1) * kSegW;
+        wgt = S.cstart[c0 + kSegW] - S.cstart[c0];
+      }
+      int rank = 0;
+#pragma unroll
+      for (int j = 0; j < kItems; ++j) {
+        const unsigned int wj = __shfl_sync(kFull, wgt, j);
+        rank += (wj > wgt || (wj == wgt && j < lane)) ? 1 : 0;
+      }
+      if (lane < kItems && wgt > 0) S.item_order[rank] = (unsigned char)lane;
+      const unsigned int nz = __ballot_sync(kFull, lane < kItems && wgt > 0);
+      if (lane == 0) S.n_items = __popc(nz);
     } else {
       // mtmp is dead from here on: its storage becomes perm, pre-filled with the dummy point
       const unsigned int fill = ((unsigned)kPCap * 16u) | (((unsigned)kMCap * 64u) << 16);
@@ -457,20 +454,13 @@ k_deposit_tile(const Params P, const Markers M, const uint32_t* __restrict__ cel
         int item = 0;
         if (lane == 0) item = atomicAdd(&S.next_item, 1);
         item = __shfl_sync(kFull, item, 0);
-        if (item >= kItems) break;
+        if (item >= S.n_items) break;
+        item = S.item_order[item];
 #ifdef ORB_PHASE_CLOCKS
         if (tid == 0) atomicAdd(d_points + 9, 1ull);
 #endif
-        // heavy items (rows owned by the tile) first, halo rows last
-        int lr, sg = item & 1;
-        if (item < kTileI * kSegs) {
-          lr = kHaloS + (item >> 1);
-        } else {
-          const int h = (item - kTileI * kSegs) >> 1;
-          lr = (h < kHaloS) ? h : kTileI + h;
-        }
+        const int lr = item >> 1, sg = item & 1;
         const int c_first = lr * kCW + sg * kSegW;
-        if (S.cstart[c_first + kSegW] == S.cstart[c_first]) continue;   // no point in the segment
         // node (row lr + a, column sg*kSegW + n), channels 2kk, 2kk+1
         double* pbase = S.tile + ((lr + a) * kNW + sg * kSegW) * 8 + 2 * kk;
         int idle = 4;   // cells since the last one that had points: >= 4 means all slots are zero
