@@ -84,6 +84,7 @@ Params make_params(const orb_grid* g, const orb_nl_policy_t* pol) {
   P.theta_map = g->desc.theta_map;
   P.eps = g->desc.a / g->desc.r0;
   P.b0 = g->desc.b0;
+  P.inv_b0 = 1.0 / g->desc.b0;
   P.rho_star = g->desc.rho_star;
   P.q = g->desc.q;
   P.nth_scale = (double)g->desc.ntheta / kTwoPi;
@@ -92,11 +93,13 @@ Params make_params(const orb_grid* g, const orb_nl_policy_t* pol) {
   P.n_fixed = 1;
   P.n_max = 1;
   P.rho_ref = 1.0;
+  P.inv_rho_ref = 1.0;
   if (pol) {
     P.adaptive = pol->mode == ORB_NL_ADAPTIVE;
     P.n_fixed = pol->n_fixed;
     P.n_max = P.adaptive ? pol->n_max : pol->n_fixed;
     P.rho_ref = P.adaptive ? pol->rho_ref : 1.0;
+    P.inv_rho_ref = 1.0 / P.rho_ref;
   }
   P.ring = g->ring;
   P.scoef = g->scoef;

@@ -121,13 +121,14 @@ struct Smem {
       atomicAdd(d_points + 2 + (i), (unsigned long long)(now__ - clk__));   \
       clk__ = now__;                                                        \
     }                                                                       \
+    __syncwarp();                                                           \
   } while (0)
 #else
 #define ORB_CLK(i) do { } while (0)
 #endif
 
 __device__ __forceinline__ void dmma884(double& c0, double& c1, double a, double b) {
-  asm("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};"
+  asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};"
                : "+d"(c0), "+d"(c1)
                : "d"(a), "d"(b));
 }
@@ -256,7 +257,7 @@ k_deposit_tile(const Params P, const Markers M, const uint32_t* __restrict__ cel
         const MarkerData m = load_marker(M, p);
         const GuidingCentre g = guiding_centre(P, m.s, m.th, m.mu);
         n = g.n;
-        const double c = P.q * m.w / (double)n;
+        const double c = P.q * m.w * __drcp_rn((double)n);
         double wp[4];
         k0 = periodic_weights(wrap_2pi(m.ph), P.nph_scale, P.nph, wp);
 #pragma unroll
@@ -275,13 +276,19 @@ k_deposit_tile(const Params P, const Markers M, const uint32_t* __restrict__ cel
       // if not, its points take the direct path
       const int k_ok = have && (k0 == k - 1);
 
-      int incl = n;
+      int incl, total;
+      if (P.adaptive || n_tile - (uint32_t)grp * 32u < 32u) {
+        incl = n;
 #pragma unroll
-      for (int o = 1; o < 32; o <<= 1) {
-        const int t = __shfl_up_sync(kFull, incl, o);
-        if (lane >= o) incl += t;
+        for (int o = 1; o < 32; o <<= 1) {
+          const int t = __shfl_up_sync(kFull, incl, o);
+          if (lane >= o) incl += t;
+        }
+        total = __shfl_sync(kFull, incl, 31);
+      } else {   // fixed N_L, full group: no scan needed
+        incl = (lane + 1) * P.n_fixed;
+        total = 32 * P.n_fixed;
       }
-      const int total = __shfl_sync(kFull, incl, 31);
 
       // capacity: marker slots first, then points (so that failed point allocations are a tail)
       unsigned int mb = 0, pb = 0;
@@ -456,9 +463,6 @@ k_deposit_tile(const Params P, const Markers M, const uint32_t* __restrict__ cel
         item = __shfl_sync(kFull, item, 0);
         if (item >= S.n_items) break;
         item = S.item_order[item];
-#ifdef ORB_PHASE_CLOCKS
-        if (tid == 0) atomicAdd(d_points + 9, 1ull);
-#endif
         const int lr = item >> 1, sg = item & 1;
         const int c_first = lr * kCW + sg * kSegW;
         // node (row lr + a, column sg*kSegW + n), channels 2kk, 2kk+1
@@ -509,6 +513,7 @@ k_deposit_tile(const Params P, const Markers M, const uint32_t* __restrict__ cel
           }                                                                          \
         }
 
+        __syncwarp();   // mma.sync.aligned below needs the whole warp converged
 #pragma unroll 1
         for (int cc = 0; cc < kSegW; cc += 4) {
           if (idle >= 4 && S.cstart[c_first + cc + 4] == S.cstart[c_first + cc]) {

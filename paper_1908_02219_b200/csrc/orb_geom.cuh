@@ -46,16 +46,16 @@ __device__ __forceinline__ GuidingCentre guiding_centre(const Params& P, double 
     const double sth = sqrt(om) * sn * inv_d;
     g.x0 = s * cth;
     g.z0 = s * sth;
-    two_mu_over_b = 2.0 * mu * om * inv_d / P.b0;   // 1/B = (1-e^2) / (B0 (1 - e cos theta*))
+    two_mu_over_b = 2.0 * mu * om * inv_d * P.inv_b0;   // 1/B = (1-e^2) / (B0 (1 - e cos theta*))
   } else {
     g.x0 = s * cs;
     g.z0 = s * sn;
-    two_mu_over_b = 2.0 * mu * fma(e, cs, 1.0) / P.b0;
+    two_mu_over_b = 2.0 * mu * fma(e, cs, 1.0) * P.inv_b0;
   }
   g.rho = P.rho_star * sqrt(two_mu_over_b);
   int n = P.n_fixed;
   if (P.adaptive) {
-    double m = ceil(g.rho / P.rho_ref);
+    double m = ceil(g.rho * P.inv_rho_ref);
     m = fmax(m, 1.0);
     double nn = fmin((double)P.n_fixed * m, (double)P.n_max);
     n = (int)nn;

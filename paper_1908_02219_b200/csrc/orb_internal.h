@@ -23,7 +23,7 @@ struct Params {
   int ns, nth, nph;      // cells
   int theta_map;
   double eps;            // a / r0
-  double b0;
+  double b0, inv_b0;
   double rho_star;
   double q;
   double nth_scale;      // ntheta / 2pi
@@ -32,7 +32,7 @@ struct Params {
   int adaptive;
   int n_fixed;           // N_L, or n_min when adaptive
   int n_max;
-  double rho_ref;
+  double rho_ref, inv_rho_ref;
   // ring table: entry (N, l) at N*(N-1)/2 + l holds (cos, sin)(alpha0 + 2 pi l / N), N = 1..ORB_MAX_NL
   const double2* ring;
   // radial spline pieces: scoef[(c*4 + a)*4 + d] = coefficient of t^d of basis c+a on cell c
