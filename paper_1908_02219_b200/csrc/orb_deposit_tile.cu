@@ -45,7 +45,10 @@
 // 16 clk per SM sub-partition (same FMA rate as DFMA) but needs one operand pair per 8 FMAs.
 // One 512-thread block per SM (v2, v3) left the SM waiting at barriers and on single-warp
 // dependency chains; three 256-thread (or two 384-thread) blocks with ~70-95 KB of shared memory
-// each overlap one tile's geometry with another's contraction and flush.
+// each overlap one tile's geometry with another's contraction and flush.  What moved the time from
+// there on was what shortens a warp's dependency chain or its wait at a barrier (phase-2 work list
+// heaviest first, reciprocals for divisions, two points in flight per lane), not what trims
+// instruction, shared-memory-wavefront or fp64-operation counts.
 #include "orb_geom.cuh"
 
 namespace orb {
@@ -66,7 +69,6 @@ constexpr int kNW = kCW + 3;               // node columns (27)
 constexpr int kCells = kCH * kCW;          // 288
 constexpr int kSegW = 12;                  // cells per walk segment
 constexpr int kSegs = kCW / kSegW;         // 2
-constexpr int kSegN = kSegW + 3;           // node columns a segment produces (15)
 constexpr int kItems = kCH * kSegs;        // 24
 constexpr int kPCap = 1536;   // Larmor points per chunk
 constexpr int kMCap = 384;    // markers per chunk
