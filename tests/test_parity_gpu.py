@@ -171,3 +171,34 @@ def test_deposit_host_roundtrip(oracle_results):
     assert npts == npts_o and up == 6 * 8 * cfg.n_markers and down == 2 * rho.nbytes
     assert_parity(rho, rho_o)
     assert_parity(jpar, jpar_o)
+
+
+@pytest.mark.parametrize("adaptive", [False, True])
+def test_nondefault_geometry_charge_field_and_gyrophase(adaptive):
+    """Every descriptor / policy field away from its default: r0, a, b0, q, rho_star, alpha0
+    (R1, R2, R6, R7, R10), fixed and adaptive N_L, all three algorithms."""
+    import torch
+    import oracle as O
+    cfg = small("cfg0", 30_011, current=True, ns=20, ntheta=40, nphi=12, r0=1.7, a=0.5, b0=2.5,
+                q=-1.5, rho_star=1 / 60.0, adaptive=adaptive, n_fixed=4 if adaptive else 6,
+                n_max=16 if adaptive else 6, s_lo=0.02, s_hi=0.98)
+    alpha0 = 0.37
+    m = W.generate(cfg)
+    og = oracle_geom(cfg)
+    op = (O.policy_adaptive(cfg.n_fixed, cfg.n_max, cfg.rho_ref, alpha0) if adaptive
+          else O.policy_fixed(cfg.n_fixed, alpha0))
+    rho_o, jpar_o, npts_o = O.deposit(og, op, *(m[f] for f in W.FIELDS), current=True)
+    d = to_device(m)
+    for flags in ALGOS.values():
+        g = B.grid_for(cfg)
+        rho = torch.zeros(g.shape(), dtype=torch.float64, device="cuda")
+        jpar = torch.zeros_like(rho)
+        g.markers_bind(d["s"], d["theta"], d["phi"], d["vpar"], d["mu"], d["w"])
+        pol = B.policy(cfg.n_fixed, adaptive=adaptive, n_max=cfg.n_max if adaptive else None,
+                       rho_ref=cfg.rho_ref, alpha0=alpha0, flags=flags)
+        g.deposit(rho, jpar, pol, torch.cuda.current_stream().cuda_stream)
+        npts = g.last_points()
+        g.destroy()
+        assert npts == npts_o
+        assert_parity(rho.cpu().numpy(), rho_o, "rho flags=%d" % flags)
+        assert_parity(jpar.cpu().numpy(), jpar_o, "jpar flags=%d" % flags)
