@@ -217,14 +217,13 @@ k_deposit_tile(const Params P, const Markers M, const uint32_t* __restrict__ cel
 #pragma unroll
     for (int d = 0; d < 8; ++d) S.mtab[kMCap * 8 + d] = 0.0;
   }
+  // (the zeroing overlaps thread 0's loads of the row offsets)
+  for (int x = tid; x <= kCells; x += kThreads) S.count[x] = 0;
+  for (int x = tid; x < kNH * kNW * 8; x += kThreads) S.tile[x] = 0.0;
   __syncthreads();
   const uint32_t n_tile = S.row_off[kTileI];
   if (n_tile == 0) return;
   const int n_groups = (int)((n_tile + 31) / 32);
-
-  for (int x = tid; x <= kCells; x += kThreads) S.count[x] = 0;
-  for (int x = tid; x < kNH * kNW * 8; x += kThreads) S.tile[x] = 0.0;
-  __syncthreads();
 
   ORB_CLK(0);   // prologue
   unsigned int my_points = 0, my_fallback = 0;
