@@ -159,6 +159,9 @@ int orb_last_fallback_points(orb_grid_t *g, int64_t *n_points);
  * marker arrays (host pointers, n doubles each; vpar may be NULL iff jpar_host is
  * NULL) to library-owned device buffers, binds, deposits into zeroed device grids
  * and copies rho (and jpar) back into the host arrays, which are OVERWRITTEN.
+ * Above 2^22 markers the work is pipelined on two library-owned streams: the markers travel in
+ * 8 slices and the copy of slice i+1 overlaps binning and deposition of slice i (the call is
+ * bound by the host link: 48 B per marker); use pinned host memory for the overlap to happen.
  * Synchronous.  Leaves the handle bound to the library's own device copies.
  * h2d_bytes / d2h_bytes (optional) receive the bytes moved. */
 int orb_deposit_host(orb_grid_t *g, int64_t n, const double *s, const double *theta,

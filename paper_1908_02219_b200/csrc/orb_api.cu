@@ -11,6 +11,10 @@
 
 using namespace orb;
 
+// orb_deposit_host pipelines the markers in this many slices: the host->device copy of slice
+// i+1 overlaps binning and deposition of slice i (the call is PCIe-bound: 48 B per marker)
+constexpr int kHostSlices = 8;
+
 struct orb_grid {
   orb_grid_desc_t desc;
   int64_t ncells;
@@ -35,6 +39,9 @@ struct orb_grid {
   double* hbuf[6];
   int64_t hbuf_capacity;
   double* hgrid[2];
+  cudaStream_t hstream[2];   // orb_deposit_host: [0] copies, [1] kernels
+  cudaEvent_t hevent[kHostSlices];
+  bool keep_counters;        // internal: next deposit adds to the point counters
 
   int64_t launches;
   char err[512];
@@ -253,6 +260,10 @@ int orb_grid_destroy(orb_grid_t* g) {
   for (int i = 0; i < 6; ++i) cudaFree(g->hbuf[i]);
   cudaFree(g->hgrid[0]);
   cudaFree(g->hgrid[1]);
+  for (int i = 0; i < 2; ++i)
+    if (g->hstream[i]) cudaStreamDestroy(g->hstream[i]);
+  for (int i = 0; i < kHostSlices; ++i)
+    if (g->hevent[i]) cudaEventDestroy(g->hevent[i]);
   cudaGetLastError();
   delete g;
   return ORB_OK;
@@ -334,7 +345,8 @@ int orb_deposit(orb_grid_t* g, double* rho, double* jpar, const orb_nl_policy_t*
     ORB_CUDA(g, cudaMemsetAsync(rho, 0, (size_t)g->nnodes * sizeof(double), st));
     if (jpar) ORB_CUDA(g, cudaMemsetAsync(jpar, 0, (size_t)g->nnodes * sizeof(double), st));
   }
-  ORB_CUDA(g, cudaMemsetAsync(g->d_points, 0, kCounters * sizeof(unsigned long long), st));
+  if (!g->keep_counters)
+    ORB_CUDA(g, cudaMemsetAsync(g->d_points, 0, kCounters * sizeof(unsigned long long), st));
 
   Params P = make_params(g, pol);
   Markers M = g->bound;
@@ -423,31 +435,58 @@ int orb_deposit_host(orb_grid_t* g, int64_t n, const double* s, const double* th
   }
   for (int i = 0; i < 2; ++i)
     if (!g->hgrid[i]) ORB_CUDA(g, cudaMalloc(&g->hgrid[i], (size_t)g->nnodes * sizeof(double)));
+  for (int i = 0; i < 2; ++i)
+    if (!g->hstream[i]) ORB_CUDA(g, cudaStreamCreateWithFlags(&g->hstream[i], cudaStreamNonBlocking));
+  for (int i = 0; i < kHostSlices; ++i)
+    if (!g->hevent[i]) ORB_CUDA(g, cudaEventCreateWithFlags(&g->hevent[i], cudaEventDisableTiming));
   const double* src[6] = {s, theta, phi, vpar, mu, w};
   int64_t up = 0, down = 0;
-  cudaStream_t st = 0;
-  for (int i = 0; i < 6; ++i) {
-    if (!src[i] || n == 0) continue;
-    ORB_CUDA(g, cudaMemcpyAsync(g->hbuf[i], src[i], (size_t)n * sizeof(double),
-                                cudaMemcpyHostToDevice, st));
-    up += n * (int64_t)sizeof(double);
+  cudaStream_t s_copy = g->hstream[0], st = g->hstream[1];
+  double* rho_d = g->hgrid[0];
+  double* jpar_d = jpar_host ? g->hgrid[1] : nullptr;
+  // slices of even length keep every slice pointer 16-byte aligned
+  const int n_slices = n >= ((int64_t)1 << 22) ? kHostSlices : 1;
+  const int64_t per = ((n + n_slices - 1) / n_slices + 1) & ~(int64_t)1;
+  if (n == 0) {
+    rc = orb_grid_zero(g, rho_d, jpar_d, st);
+    if (rc != ORB_OK) return rc;
+    ORB_CUDA(g, cudaMemsetAsync(g->d_points, 0, kCounters * sizeof(unsigned long long), st));
   }
-  rc = orb_markers_bind(g, n, g->hbuf[0], g->hbuf[1], g->hbuf[2], vpar ? g->hbuf[3] : nullptr,
-                        g->hbuf[4], g->hbuf[5], 0);
-  if (rc != ORB_OK) return rc;
-  orb_nl_policy_t p2 = *pol;
-  p2.flags |= ORB_DEPOSIT_ZERO_FIRST;
-  rc = orb_deposit(g, g->hgrid[0], jpar_host ? g->hgrid[1] : nullptr, &p2, st);
-  if (rc != ORB_OK) return rc;
-  ORB_CUDA(g, cudaMemcpyAsync(rho_host, g->hgrid[0], (size_t)g->nnodes * sizeof(double),
+  for (int i = 0; i < n_slices && n > 0; ++i) {
+    const int64_t off = i * per;
+    const int64_t len = (off + per <= n ? per : n - off);
+    if (len <= 0) break;
+    for (int f = 0; f < 6; ++f) {
+      if (!src[f]) continue;
+      ORB_CUDA(g, cudaMemcpyAsync(g->hbuf[f] + off, src[f] + off, (size_t)len * sizeof(double),
+                                  cudaMemcpyHostToDevice, s_copy));
+      up += len * (int64_t)sizeof(double);
+    }
+    ORB_CUDA(g, cudaEventRecord(g->hevent[i], s_copy));
+    ORB_CUDA(g, cudaStreamWaitEvent(st, g->hevent[i], 0));
+    rc = orb_markers_bind(g, len, g->hbuf[0] + off, g->hbuf[1] + off, g->hbuf[2] + off,
+                          vpar ? g->hbuf[3] + off : nullptr, g->hbuf[4] + off, g->hbuf[5] + off, 0);
+    if (rc != ORB_OK) return rc;
+    orb_nl_policy_t p2 = *pol;
+    if (i == 0) p2.flags |= ORB_DEPOSIT_ZERO_FIRST; else p2.flags &= ~ORB_DEPOSIT_ZERO_FIRST;
+    g->keep_counters = i > 0;
+    rc = orb_deposit(g, rho_d, jpar_d, &p2, st);
+    g->keep_counters = false;
+    if (rc != ORB_OK) return rc;
+  }
+  ORB_CUDA(g, cudaMemcpyAsync(rho_host, rho_d, (size_t)g->nnodes * sizeof(double),
                               cudaMemcpyDeviceToHost, st));
   down += g->nnodes * (int64_t)sizeof(double);
   if (jpar_host) {
-    ORB_CUDA(g, cudaMemcpyAsync(jpar_host, g->hgrid[1], (size_t)g->nnodes * sizeof(double),
+    ORB_CUDA(g, cudaMemcpyAsync(jpar_host, jpar_d, (size_t)g->nnodes * sizeof(double),
                                 cudaMemcpyDeviceToHost, st));
     down += g->nnodes * (int64_t)sizeof(double);
   }
   ORB_CUDA(g, cudaStreamSynchronize(st));
+  // leave the handle bound to the whole device copy (not binned)
+  rc = orb_markers_bind(g, n, g->hbuf[0], g->hbuf[1], g->hbuf[2], vpar ? g->hbuf[3] : nullptr,
+                        g->hbuf[4], g->hbuf[5], 0);
+  if (rc != ORB_OK) return rc;
   if (n_points) {
     unsigned long long v = 0;
     ORB_CUDA(g, cudaMemcpy(&v, g->d_points, sizeof(v), cudaMemcpyDeviceToHost));

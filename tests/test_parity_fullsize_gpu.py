@@ -137,3 +137,24 @@ def test_cfg4_presorted_sampled_planes(cfg4_case):
     assert npts == npts_o
     _check_planes(rho, jpar, planes)
     _conservation(cfg, m, rho, jpar)
+
+
+def test_deposit_host_sliced_pipeline():
+    """orb_deposit_host above 2^22 markers: host->device copies in slices overlapped with binning
+    and deposition of the previous slice; result and point count must not depend on the slicing."""
+    import dataclasses
+    cfg = dataclasses.replace(W.scaled(W.CONFIGS["cfg4"], (1 << 22) + 12_345), ns=64, ntheta=128,
+                              nphi=32, rho_star=1 / 120.0)
+    m = W.generate(cfg)
+    rho_o, jpar_o, npts_o, _ = O.deposit_ranges(oracle_geom(cfg), oracle_policy(cfg),
+                                                *(m[f] for f in W.FIELDS), current=True)
+    g = B.grid_for(cfg)
+    rho = np.empty((cfg.ns + 3, cfg.ntheta, cfg.nphi))
+    jpar = np.empty_like(rho)
+    for _ in range(2):      # second call reuses streams, events and scratch
+        npts, up, down = g.deposit_host(m["s"], m["theta"], m["phi"], m["vpar"], m["mu"], m["w"],
+                                        rho, jpar, B.policy_for(cfg))
+        assert npts == npts_o and up == 6 * 8 * cfg.n_markers and down == 2 * rho.nbytes
+        assert rel_err(rho, rho_o) <= TOL
+        assert rel_err(jpar, jpar_o) <= TOL
+    g.destroy()
