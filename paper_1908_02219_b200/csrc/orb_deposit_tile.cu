@@ -512,6 +512,7 @@ k_deposit_tile(const Params P, const Markers M, const uint32_t* __restrict__ cel
               c1a = 0.0; c1b = 0.0;                                                  \
             }                                                                        \
           }                                                                          \
+          __syncwarp();   /* the CAS loops diverge; mma.sync.aligned needs the warp whole */ \
         }
 
         __syncwarp();   // mma.sync.aligned below needs the whole warp converged
