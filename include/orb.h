@@ -184,6 +184,12 @@ int orb_launch_count(const orb_grid_t *g, int64_t *n_launches);
  * of basis function c+a on radial cell c.  ORB_E_INVAL if ns < 4 or out is NULL. */
 int orb_spline_table_radial(int32_t ns, double *out);
 
+/* Harness aid, not part of the hot path: measures the fp64 FMA rate of `device` (8 independent
+ * DFMA chains per thread, 4 x 512 threads per SM, one timed launch after a warm-up) and writes it
+ * as TFLOP/s (2 flop per FMA).  The deposition is bound by the fp64 pipe, so this is the roof
+ * bench.py reports `roofline_alu` against.  Synchronous; takes a few milliseconds. */
+int orb_probe_dfma(int32_t device, double *tflops);
+
 /* Static text for a status code. */
 const char *orb_strerror(int code);
 

@@ -22,7 +22,7 @@ ORB_MAX_NL = 32
 # every symbol include/orb.h declares
 SYMBOLS = ("orb_grid_create", "orb_grid_destroy", "orb_grid_shape", "orb_markers_bind",
            "orb_markers_bin", "orb_deposit", "orb_grid_zero", "orb_last_points", "orb_last_fallback_points", "orb_deposit_host",
-           "orb_launch_count", "orb_debug_counters", "orb_spline_table_radial", "orb_strerror", "orb_last_error", "orb_version")
+           "orb_launch_count", "orb_debug_counters", "orb_probe_dfma", "orb_spline_table_radial", "orb_strerror", "orb_last_error", "orb_version")
 
 
 class OrbError(RuntimeError):
@@ -102,6 +102,13 @@ def _ptr(t):
 def policy(n_fixed=4, *, adaptive=False, n_max=None, rho_ref=1.0, alpha0=0.0, flags=0) -> NlPolicy:
     return NlPolicy(ORB_NL_ADAPTIVE if adaptive else ORB_NL_FIXED, n_fixed,
                     n_max if n_max is not None else n_fixed, flags, rho_ref, alpha0)
+
+
+def probe_dfma(device: int = 0) -> float:
+    """Measured fp64 FMA rate of the device, TFLOP/s (harness aid)."""
+    v = C.c_double()
+    _check(lib().orb_probe_dfma(device, C.byref(v)))
+    return v.value
 
 
 def spline_table_radial(ns: int):

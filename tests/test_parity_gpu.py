@@ -202,3 +202,13 @@ def test_nondefault_geometry_charge_field_and_gyrophase(adaptive):
         assert npts == npts_o
         assert_parity(rho.cpu().numpy(), rho_o, "rho flags=%d" % flags)
         assert_parity(jpar.cpu().numpy(), jpar_o, "jpar flags=%d" % flags)
+
+
+def test_fp64_probe_is_plausible():
+    """orb_probe_dfma (the roof bench.py reports roofline_alu against): between half and 1.2x of
+    the nominal SMs x 64 lanes x 2 flop x clock."""
+    import torch
+    p = torch.cuda.get_device_properties(0)
+    nominal = p.multi_processor_count * 64 * 2 * (p.clock_rate * 1e3 if hasattr(p, "clock_rate") else 1.965e9) / 1e12
+    got = B.probe_dfma(0)
+    assert 0.5 * nominal < got < 1.2 * nominal, (got, nominal)
