@@ -70,7 +70,9 @@ constexpr int kCells = kCH * kCW;          // 288
 constexpr int kSegW = 12;                  // cells per walk segment
 constexpr int kSegs = kCW / kSegW;         // 2
 constexpr int kItems = kCH * kSegs;        // 24
-constexpr int kPCap = 1536;   // Larmor points per chunk
+constexpr int kPCap = 2304;   // Larmor points per chunk: 6 per marker slot, so that adaptive N_L
+                              // (mean ~7 points per marker) fills the marker slots too; with
+                              // fixed N_L = 4 the marker cap binds (1536 points)
 constexpr int kMCap = 384;    // markers per chunk
 constexpr int kPermCap = kPCap + 3 * kCells;   // points + padding to batches of 4
 constexpr unsigned kFull = 0xffffffffu;
