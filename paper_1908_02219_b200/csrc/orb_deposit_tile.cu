@@ -70,17 +70,19 @@ constexpr int kCells = kCH * kCW;          // 288
 constexpr int kSegW = 12;                  // cells per walk segment
 constexpr int kSegs = kCW / kSegW;         // 2
 constexpr int kItems = kCH * kSegs;        // 24
-constexpr int kPCap = 2304;   // Larmor points per chunk: 6 per marker slot, so that adaptive N_L
-                              // (mean ~7 points per marker) fills the marker slots too; with
-                              // fixed N_L = 4 the marker cap binds (1536 points)
 constexpr int kMCap = 384;    // markers per chunk
-constexpr int kPermCap = kPCap + 3 * kCells;   // points + padding to batches of 4
+// Larmor points per chunk, a template parameter (PCAP) of the kernel: 4 per marker slot when
+// N_L <= 4 is fixed (the marker cap binds), 6 per marker slot otherwise, so that adaptive N_L (mean
+// ~7 points per marker) fills the marker slots too.  The small variant leaves 30 KB more of the
+// SM's 228 KB to L1.
+constexpr int kPCapSmall = 1536;
+constexpr int kPCapLarge = 2304;
 constexpr unsigned kFull = 0xffffffffu;
 constexpr unsigned kNoCell = 0x1ffu;       // meta cell field of a point deposited directly
 static_assert(kCW % kSegW == 0 && kSegW % 4 == 0, "segments must tile the row in groups of 4");
-static_assert(kPCap >= 32 * ORB_MAX_NL && kPCap < 4096 && kMCap % 32 == 0 && kMCap < 2047, "caps");
+static_assert(kPCapSmall >= 32 * ORB_MAX_NL && kPCapLarge < 4096 && kMCap % 32 == 0 && kMCap < 2047, "caps");
 static_assert(kCells < (int)kNoCell, "cell id must fit 9 bits");
-static_assert(kPCap * 16 < 65536 && kMCap * 64 < 65536, "perm entries hold 16-bit byte offsets");
+static_assert(kPCapLarge * 16 < 65536 && kMCap * 64 < 65536, "perm entries hold 16-bit byte offsets");
 
 // meta word of a point slot.  After phase 1a: marker slot << 21 | point index in the ring.
 // After phase 1b: marker slot << 21 | rank inside the cell << 9 | tile-local cell.
@@ -93,8 +95,10 @@ struct MarkerTmp {      // phase 1a -> 1b hand-over, 32 bytes
   int k0;               // first phi node (phi cell - 1)
 };
 
-template <int G>
+template <int G, int PCAP>
 struct Smem {
+  static constexpr int kPCap = PCAP;
+  static constexpr int kPermCap = PCAP + 3 * kCells;   // points + padding to batches of 4
   double tile[kNH * kNW * 8];            // [node row][node col][grid*4 + phi plane]
   double2 rec[kPCap + 1];                // (t_s, t_theta) of a Larmor point; [kPCap] = dummy
   double mtab[(kMCap + 1) * 8];          // per marker: c*wphi[0..3], c*vpar*wphi[0..3]; [kMCap] = dummy (zeros)
@@ -173,13 +177,15 @@ __device__ __noinline__ void deposit_point_global(const Params& P, double s_l, d
   }
 }
 
-template <int G>   // G = 1: rho only; G = 2: rho and jpar
+template <int G, int PCAP>   // G = 1: rho only; G = 2: rho and jpar; PCAP: points per chunk
 __global__ void __launch_bounds__(kThreads, kCtasPerSm)
 k_deposit_tile(const Params P, const Markers M, const uint32_t* __restrict__ cell_start,
                double* __restrict__ rho, double* __restrict__ jpar,
                unsigned long long* __restrict__ d_points, int tiles_i, int tiles_j) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
-  Smem<G>& S = *reinterpret_cast<Smem<G>*>(smem_raw);
+  Smem<G, PCAP>& S = *reinterpret_cast<Smem<G, PCAP>*>(smem_raw);
+  constexpr int kPCap = PCAP;
+  constexpr int kPermCap = Smem<G, PCAP>::kPermCap;
 
   const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
 #ifdef ORB_PHASE_CLOCKS
@@ -602,18 +608,18 @@ k_deposit_tile(const Params P, const Markers M, const uint32_t* __restrict__ cel
   }
 }
 
-template <int G>
+template <int G, int PCAP>
 int launch(const Params& P, const Markers& M, const uint32_t* cell_start, double* rho, double* jpar,
            unsigned long long* d_points, cudaStream_t st) {
   const int tiles_i = (P.ns + kTileI - 1) / kTileI;
   const int tiles_j = (P.nth + kTileJ - 1) / kTileJ;
   const dim3 blocks((unsigned)tiles_j, (unsigned)tiles_i, (unsigned)P.nph);
-  const size_t smem = sizeof(Smem<G>);
-  if (cudaFuncSetAttribute(k_deposit_tile<G>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+  const size_t smem = sizeof(Smem<G, PCAP>);
+  if (cudaFuncSetAttribute(k_deposit_tile<G, PCAP>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                            (int)smem) != cudaSuccess)
     return -1;
-  k_deposit_tile<G><<<blocks, kThreads, smem, st>>>(P, M, cell_start, rho, jpar,
-                                                                   d_points, tiles_i, tiles_j);
+  k_deposit_tile<G, PCAP><<<blocks, kThreads, smem, st>>>(P, M, cell_start, rho, jpar, d_points,
+                                                         tiles_i, tiles_j);
   return 1;
 }
 
@@ -622,8 +628,11 @@ int launch(const Params& P, const Markers& M, const uint32_t* cell_start, double
 int launch_deposit_tile(const Params& P, const Markers& M, const uint32_t* cell_start, double* rho,
                         double* jpar, unsigned long long* d_points, cudaStream_t st) {
   if (M.n == 0) return 0;
-  return jpar ? launch<2>(P, M, cell_start, rho, jpar, d_points, st)
-              : launch<1>(P, M, cell_start, rho, jpar, d_points, st);
+  if (!P.adaptive && P.n_fixed <= 4)
+    return jpar ? launch<2, kPCapSmall>(P, M, cell_start, rho, jpar, d_points, st)
+                : launch<1, kPCapSmall>(P, M, cell_start, rho, jpar, d_points, st);
+  return jpar ? launch<2, kPCapLarge>(P, M, cell_start, rho, jpar, d_points, st)
+              : launch<1, kPCapLarge>(P, M, cell_start, rho, jpar, d_points, st);
 }
 
 }  // namespace orb
