@@ -50,7 +50,7 @@ FP64_NOMINAL_TFLOPS = 37.2
 
 # dram__bytes_read.sum + dram__bytes_write.sum of ONE launch of the deposit kernel, from the
 # `ncu --set full` capture summarised in profiles/ (None until a capture of that workload exists)
-NCU_TRAFFIC_BYTES = {"cfg3": 5074429000 + 757326592}   # profiles/r01_final_deposit_ncu.md
+NCU_TRAFFIC_BYTES = {"cfg3": 5075555000 + 758216192}   # profiles/r01_final_deposit_ncu.md
 
 
 def measured_hbm_peak():
