@@ -335,7 +335,9 @@ def run_ours(args):
                          "peak": peak, "unit": "GB/s", "frac": achieved / peak,
                          "traffic": NCU_TRAFFIC_BYTES.get(cfg.name), "peak_source": peak_src,
                          "algorithmic_bytes": alg_bytes, "kernel_ms": dep_ms,
-                         "frac_of_nominal_8TBs": achieved / HBM_NOMINAL_GBS},
+                         "frac_of_nominal_8TBs": achieved / HBM_NOMINAL_GBS,
+                         "note": "contract metric of BASELINE.json; the roof that actually binds "
+                                 "this path is the fp64 pipe: see roofline_alu (DESIGN.md 6)"},
             "roofline_alu": {"bound": "alu", "pipe": "fp64", "kernel": "k_deposit_tile",
                              "achieved": flops / (dep_ms * 1e-3) / 1e12, "peak": fp64_peak,
                              "peak_source": fp64_src,
