@@ -33,8 +33,11 @@
  *   - "device pointer" = memory of the CUDA device given in the descriptor
  *     (e.g. torch.Tensor.data_ptr()); "host pointer" = ordinary host memory.
  *   - `stream` is a cudaStream_t passed as void* (NULL = legacy default stream).
- *     Calls that take a stream only enqueue work on it and do not synchronise
- *     the host, unless stated.
+ *     Calls that take a stream only enqueue work on it; they neither synchronise
+ *     the host nor allocate, so a sequence orb_markers_bin / orb_grid_zero /
+ *     orb_deposit can be captured into a CUDA graph.  A handle keeps state between
+ *     calls (binned order, ring table, counters): issue the calls of one handle to
+ *     ONE stream, or order the streams yourself (events) -- the library does not.
  *   - there is no CPU fallback: without a usable CUDA device orb_grid_create
  *     fails with ORB_E_CUDA.
  */
@@ -82,6 +85,9 @@ enum { ORB_NL_FIXED = 0, ORB_NL_ADAPTIVE = 1 };
 #define ORB_DEPOSIT_ALGO_ATOMIC 0x4u /* use the one-thread-per-marker global-atomics kernel
                                         (the GPU algorithm of) instead of the
                                         shared-memory tile kernel                              */
+#define ORB_DEPOSIT_ALGO_TILE_V4 0x8u /* use the round-1 tile kernel (one block per tile, all
+                                        warps run all phases) instead of the persistent
+                                        warp-specialised one; kept for comparison               */
 
 /* Number of Larmor points per marker (R7-R9):
  *   FIXED:    N_L = n_fixed
@@ -119,16 +125,24 @@ int orb_grid_shape(const orb_grid_t *g, int64_t dims[3]);
  * BORROWED: no copy is made; they must stay valid and unmodified until the next
  * bind or destroy, and the library never writes to them.  vpar may be NULL if
  * jpar will always be NULL.  Pointers must be 16-byte aligned.  Marker VALUES are
- * not validated.  Any previous binning is discarded.  n = 0 is legal. */
+ * not validated; s outside [0,1] is treated as the nearest bound (R11).  Any
+ * previous binning is discarded.  n = 0 is legal.
+ * Unless ORB_MARKERS_SORTED is given, bind makes sure the binning scratch (68 bytes
+ * per marker) can hold n markers; growing it allocates device memory, which
+ * synchronises the device -- call orb_reserve first to keep bind allocation-free. */
 int orb_markers_bind(orb_grid_t *g, int64_t n, const double *s, const double *theta,
                      const double *phi, const double *vpar, const double *mu, const double *w,
                      uint32_t flags);
+
+/* Pre-allocates the marker-proportional scratch for up to n markers (ORB_E_NOMEM if the
+ * device cannot hold it).  Optional: orb_markers_bind grows it on demand. */
+int orb_reserve(orb_grid_t *g, int64_t n);
 
 /* Runs (or refreshes) the binning pass alone on `stream`, so that it can be timed
  * apart from the deposit (BASELINE.json config 4; the bucket sort of PAPER.md:167):
  * counting sort of the bound markers by guiding-centre cell into library-owned
  * scratch.  For ORB_MARKERS_SORTED bindings only the per-cell offsets are built.
- * May allocate scratch on first use (which synchronises); afterwards asynchronous. */
+ * Asynchronous; never allocates. */
 int orb_markers_bin(orb_grid_t *g, void *stream);
 
 /* Adds the charge density into rho and, if jpar != NULL, the parallel current
@@ -146,7 +160,8 @@ int orb_deposit(orb_grid_t *g, double *rho, double *jpar, const orb_nl_policy_t 
 int orb_grid_zero(orb_grid_t *g, double *rho, double *jpar, void *stream);
 
 /* Sum of N_L over the markers of the last orb_deposit on this handle.
- * Synchronises with that deposit (one 8-byte device-to-host copy). */
+ * Waits for that deposit only (an event recorded on its stream; if the deposit was
+ * captured into a CUDA graph, for the whole device) and copies 8 bytes back. */
 int orb_last_points(orb_grid_t *g, int64_t *n_points);
 
 /* Of those, the Larmor points of the last orb_deposit whose 4x4 (s, theta*) footprint left the

@@ -16,12 +16,13 @@ ORB_NL_FIXED, ORB_NL_ADAPTIVE = 0, 1
 ORB_DEPOSIT_ZERO_FIRST = 0x1
 ORB_DEPOSIT_NO_BIN = 0x2
 ORB_DEPOSIT_ALGO_ATOMIC = 0x4
+ORB_DEPOSIT_ALGO_TILE_V4 = 0x8
 ORB_MARKERS_SORTED = 0x1
 ORB_MAX_NL = 32
 
 # every symbol include/orb.h declares
 SYMBOLS = ("orb_grid_create", "orb_grid_destroy", "orb_grid_shape", "orb_markers_bind",
-           "orb_markers_bin", "orb_deposit", "orb_grid_zero", "orb_last_points", "orb_last_fallback_points", "orb_deposit_host",
+           "orb_reserve", "orb_markers_bin", "orb_deposit", "orb_grid_zero", "orb_last_points", "orb_last_fallback_points", "orb_deposit_host",
            "orb_launch_count", "orb_debug_counters", "orb_probe_dfma", "orb_spline_table_radial", "orb_strerror", "orb_last_error", "orb_version")
 
 
@@ -60,6 +61,7 @@ def lib():
     L.orb_grid_destroy.argtypes = [vp]
     L.orb_grid_shape.argtypes = [vp, C.POINTER(C.c_int64 * 3)]
     L.orb_markers_bind.argtypes = [vp, C.c_int64, dp, dp, dp, dp, dp, dp, C.c_uint32]
+    L.orb_reserve.argtypes = [vp, C.c_int64]
     L.orb_markers_bin.argtypes = [vp, vp]
     L.orb_deposit.argtypes = [vp, dp, dp, C.POINTER(NlPolicy), vp]
     L.orb_grid_zero.argtypes = [vp, dp, dp, vp]
@@ -140,6 +142,9 @@ class Grid:
         self._keep = (s, theta, phi, vpar, mu, w)   # the library borrows the pointers
         _check(lib().orb_markers_bind(self._h, n, _ptr(s), _ptr(theta), _ptr(phi), _ptr(vpar),
                                       _ptr(mu), _ptr(w), flags), self._h)
+
+    def reserve(self, n):
+        _check(lib().orb_reserve(self._h, n), self._h)
 
     def markers_bin(self, stream=None):
         _check(lib().orb_markers_bin(self._h, stream), self._h)

@@ -34,6 +34,9 @@ struct orb_grid {
   double ring_alpha0;
   bool ring_valid;
   unsigned long long* d_points;
+  cudaEvent_t dep_event;     // recorded after the last deposit (orb_last_points waits on it)
+  bool dep_event_valid;
+  int sms;                   // multiprocessors of the device
 
   // orb_deposit_host staging (owned)
   double* hbuf[6];
@@ -129,19 +132,13 @@ int check_policy(orb_grid* g, const orb_nl_policy_t* pol) {
   return ORB_OK;
 }
 
-// (cos, sin)(alpha0 + 2 pi l / N) for N = 1..ORB_MAX_NL, l < N; entry at N(N-1)/2 + l.
+// (cos, sin)(alpha0 + 2 pi l / N) for N = 1..ORB_MAX_NL, l < N; entry at N(N-1)/2 + l.  Built by a
+// one-block kernel on the caller's stream (no host synchronisation, capturable in a CUDA graph).
 int upload_ring(orb_grid* g, double alpha0, cudaStream_t st) {
   if (g->ring_valid && g->ring_alpha0 == alpha0) return ORB_OK;
-  const int total = ORB_MAX_NL * (ORB_MAX_NL + 1) / 2;
-  std::vector<double2> h(total);
-  for (int n = 1; n <= ORB_MAX_NL; ++n)
-    for (int l = 0; l < n; ++l) {
-      const double al = alpha0 + kTwoPi * (double)l / (double)n;
-      h[n * (n - 1) / 2 + l] = make_double2(cos(al), sin(al));
-    }
-  // pageable source: the copy is staged before the call returns
-  ORB_CUDA(g, cudaMemcpyAsync(g->ring, h.data(), total * sizeof(double2), cudaMemcpyHostToDevice, st));
-  ORB_CUDA(g, cudaStreamSynchronize(st));
+  int l = launch_ring_table(g->ring, alpha0, st);
+  if (l < 0) return fail(g, ORB_E_CUDA, "ring table launch", cudaGetLastError());
+  g->launches += l;
   g->ring_alpha0 = alpha0;
   g->ring_valid = true;
   return ORB_OK;
@@ -155,16 +152,17 @@ void free_bin(orb_grid* g) {
   g->bin_capacity = 0;
 }
 
-int ensure_bin_scratch(orb_grid* g, int64_t n, bool need_records) {
-  if (!g->bin.cell_start) {
-    ORB_CUDA(g, cudaMalloc(&g->bin.cell_start, (size_t)(g->ncells + 1) * sizeof(uint32_t)));
-    const int64_t nb = (g->ncells + 4095) / 4096 + 1;
-    ORB_CUDA(g, cudaMalloc(&g->bin.block_sums, (size_t)nb * sizeof(uint32_t)));
-  }
-  if (need_records && n > g->bin_capacity) {
+// marker-proportional scratch (rank + binned records); called from orb_markers_bind / orb_reserve
+// only, so that orb_markers_bin and orb_deposit never allocate (cudaMalloc synchronises)
+int ensure_bin_scratch(orb_grid* g, int64_t n) {
+  if (n > g->bin_capacity) {
     free_bin(g);
     ORB_CUDA(g, cudaMalloc(&g->bin.rank, (size_t)n * sizeof(uint32_t)));
-    ORB_CUDA(g, cudaMalloc(&g->bin.rec, (size_t)n * kRecDoubles * sizeof(double)));
+    if (cudaMalloc(&g->bin.rec, (size_t)n * kRecDoubles * sizeof(double)) != cudaSuccess) {
+      cudaGetLastError();
+      free_bin(g);
+      return fail(g, ORB_E_NOMEM, "binned-record scratch");
+    }
     g->bin_capacity = n;
   }
   return ORB_OK;
@@ -172,8 +170,8 @@ int ensure_bin_scratch(orb_grid* g, int64_t n, bool need_records) {
 
 int do_bin(orb_grid* g, cudaStream_t st) {
   const bool presorted = (g->bind_flags & ORB_MARKERS_SORTED) != 0;
-  int rc = ensure_bin_scratch(g, g->bound.n, !presorted);
-  if (rc != ORB_OK) return rc;
+  if (!presorted && g->bound.n > g->bin_capacity)
+    return fail(g, ORB_E_STATE, "binning scratch missing (bind allocates it)");
   Params P = make_params(g, nullptr);
   Markers M = g->bound;
   M.rec = nullptr;
@@ -183,6 +181,11 @@ int do_bin(orb_grid* g, cudaStream_t st) {
   ORB_CUDA(g, cudaGetLastError());
   g->binned = true;
   return ORB_OK;
+}
+
+// host wait for the last deposit enqueued on this handle
+cudaError_t wait_deposit(orb_grid* g) {
+  return g->dep_event_valid ? cudaEventSynchronize(g->dep_event) : cudaDeviceSynchronize();
 }
 
 }  // namespace
@@ -213,6 +216,8 @@ int orb_grid_create(const orb_grid_desc_t* d, orb_grid_t** out) {
   const int64_t ncells = (int64_t)d->ns * d->ntheta * d->nphi;
   const int64_t nnodes = (int64_t)(d->ns + 3) * d->ntheta * d->nphi;
   if (ncells >= (int64_t)1 << 31) return ORB_E_INVAL;
+  // launch-grid limits of the tile kernels (65535 blocks along y and z)
+  if (d->nphi > 65535 || (d->ns + 7) / 8 > 65535) return ORB_E_INVAL;
   int ndev = 0;
   if (cudaGetDeviceCount(&ndev) != cudaSuccess || d->device < 0 || d->device >= ndev) {
     cudaGetLastError();
@@ -235,11 +240,19 @@ int orb_grid_create(const orb_grid_desc_t* d, orb_grid_t** out) {
           cudaSuccess ||
       cudaMalloc(&g->ring, total * sizeof(double2)) != cudaSuccess ||
       cudaMalloc(&g->d_points, kCounters * sizeof(unsigned long long)) != cudaSuccess ||
-      cudaMemset(g->d_points, 0, kCounters * sizeof(unsigned long long)) != cudaSuccess) {
+      cudaMemset(g->d_points, 0, kCounters * sizeof(unsigned long long)) != cudaSuccess ||
+      cudaMalloc(&g->bin.cell_start, (size_t)(ncells + 1) * sizeof(uint32_t)) != cudaSuccess ||
+      cudaMalloc(&g->bin.block_sums, (size_t)((ncells + 4095) / 4096 + 1) * sizeof(uint32_t)) !=
+          cudaSuccess ||
+      cudaEventCreateWithFlags(&g->dep_event, cudaEventDisableTiming) != cudaSuccess ||
+      cudaDeviceGetAttribute(&g->sms, cudaDevAttrMultiProcessorCount, d->device) != cudaSuccess) {
     cudaGetLastError();
     cudaFree(g->scoef);
     cudaFree(g->ring);
     cudaFree(g->d_points);
+    cudaFree(g->bin.cell_start);
+    cudaFree(g->bin.block_sums);
+    if (g->dep_event) cudaEventDestroy(g->dep_event);
     delete g;
     return ORB_E_CUDA;
   }
@@ -264,6 +277,7 @@ int orb_grid_destroy(orb_grid_t* g) {
     if (g->hstream[i]) cudaStreamDestroy(g->hstream[i]);
   for (int i = 0; i < kHostSlices; ++i)
     if (g->hevent[i]) cudaEventDestroy(g->hevent[i]);
+  if (g->dep_event) cudaEventDestroy(g->dep_event);
   cudaGetLastError();
   delete g;
   return ORB_OK;
@@ -296,6 +310,12 @@ int orb_markers_bind(orb_grid_t* g, int64_t n, const double* s, const double* th
   if (!aligned16(s) || !aligned16(theta) || !aligned16(phi) || !aligned16(vpar) ||
       !aligned16(mu) || !aligned16(w))
     return fail(g, ORB_E_INVAL, "marker arrays must be 16-byte aligned");
+  if (!(flags & ORB_MARKERS_SORTED) && n > g->bin_capacity) {
+    DeviceGuard dg(g->desc.device);
+    if (!dg.ok) return fail(g, ORB_E_CUDA, "cudaSetDevice");
+    int rc = ensure_bin_scratch(g, n);
+    if (rc != ORB_OK) return rc;
+  }
   g->bound.s = s;
   g->bound.th = theta;
   g->bound.ph = phi;
@@ -309,6 +329,14 @@ int orb_markers_bind(orb_grid_t* g, int64_t n, const double* s, const double* th
   g->binned = false;
   g->err[0] = 0;
   return ORB_OK;
+}
+
+int orb_reserve(orb_grid_t* g, int64_t n) {
+  if (!g) return ORB_E_INVAL;
+  if (n < 0 || n >= ((int64_t)1 << 32) - 1) return fail(g, ORB_E_INVAL, "n out of range");
+  DeviceGuard dg(g->desc.device);
+  if (!dg.ok) return fail(g, ORB_E_CUDA, "cudaSetDevice");
+  return ensure_bin_scratch(g, n);
 }
 
 int orb_markers_bin(orb_grid_t* g, void* stream) {
@@ -336,6 +364,7 @@ int orb_deposit(orb_grid_t* g, double* rho, double* jpar, const orb_nl_policy_t*
   rc = upload_ring(g, pol->alpha0, st);
   if (rc != ORB_OK) return rc;
   const bool atomic_algo = (pol->flags & ORB_DEPOSIT_ALGO_ATOMIC) != 0;
+  const bool tile_v4 = (pol->flags & ORB_DEPOSIT_ALGO_TILE_V4) != 0;
   const bool no_bin = (pol->flags & ORB_DEPOSIT_NO_BIN) != 0;
   if (!no_bin && !atomic_algo && !g->binned) {
     rc = do_bin(g, st);
@@ -356,12 +385,24 @@ int orb_deposit(orb_grid_t* g, double* rho, double* jpar, const orb_nl_policy_t*
   int l;
   if (atomic_algo || !use_binned) {
     l = launch_deposit_atomic(P, M, rho, jpar, g->d_points, st);
-  } else {
+  } else if (tile_v4) {
     l = launch_deposit_tile(P, M, g->bin.cell_start, rho, jpar, g->d_points, st);
+  } else {
+    l = launch_deposit_ws(P, M, g->bin.cell_start, rho, jpar, g->d_points, g->sms, st);
   }
   if (l < 0) return fail(g, ORB_E_CUDA, "deposit launch", cudaGetLastError());
   g->launches += l;
   ORB_CUDA(g, cudaGetLastError());
+  // orb_last_points waits on this event; an event cannot be waited on from the host while its
+  // stream is being captured into a graph, so then the device-wide wait is used instead
+  cudaStreamCaptureStatus cap = cudaStreamCaptureStatusNone;
+  if (cudaStreamIsCapturing(st, &cap) != cudaSuccess) cudaGetLastError();
+  if (cap == cudaStreamCaptureStatusNone) {
+    ORB_CUDA(g, cudaEventRecord(g->dep_event, st));
+    g->dep_event_valid = true;
+  } else {
+    g->dep_event_valid = false;
+  }
   return ORB_OK;
 }
 
@@ -380,8 +421,7 @@ int orb_last_points(orb_grid_t* g, int64_t* n_points) {
   if (!g || !n_points) return ORB_E_INVAL;
   DeviceGuard dg(g->desc.device);
   unsigned long long v = 0;
-  // default-stream copy: waits for prior work on blocking streams; then make sure
-  ORB_CUDA(g, cudaDeviceSynchronize());
+  ORB_CUDA(g, wait_deposit(g));
   ORB_CUDA(g, cudaMemcpy(&v, g->d_points, sizeof(v), cudaMemcpyDeviceToHost));
   *n_points = (int64_t)v;
   return ORB_OK;
@@ -391,7 +431,7 @@ int orb_last_fallback_points(orb_grid_t* g, int64_t* n_points) {
   if (!g || !n_points) return ORB_E_INVAL;
   DeviceGuard dg(g->desc.device);
   unsigned long long v = 0;
-  ORB_CUDA(g, cudaDeviceSynchronize());
+  ORB_CUDA(g, wait_deposit(g));
   ORB_CUDA(g, cudaMemcpy(&v, g->d_points + 1, sizeof(v), cudaMemcpyDeviceToHost));
   *n_points = (int64_t)v;
   return ORB_OK;
@@ -400,7 +440,7 @@ int orb_last_fallback_points(orb_grid_t* g, int64_t* n_points) {
 int orb_debug_counters(orb_grid_t* g, uint64_t out[16]) {
   if (!g || !out) return ORB_E_INVAL;
   DeviceGuard dg(g->desc.device);
-  ORB_CUDA(g, cudaDeviceSynchronize());
+  ORB_CUDA(g, wait_deposit(g));
   ORB_CUDA(g, cudaMemcpy(out, g->d_points, kCounters * sizeof(unsigned long long),
                          cudaMemcpyDeviceToHost));
   return ORB_OK;

@@ -18,6 +18,7 @@ struct GuidingCentre {
   double s, ts;    // s, wrapped theta* in [0, 2pi]
   double x0, z0;   // position in the poloidal plane relative to the axis, units of a
   double rho;      // Larmor radius, units of a
+  double cg, sg;   // cos, sin of the wrapped theta*
   int n;           // N_L
 };
 
@@ -29,6 +30,7 @@ __device__ __forceinline__ double wrap_2pi(double u) {
 __device__ __forceinline__ GuidingCentre guiding_centre(const Params& P, double s, double th,
                                                         double mu) {
   GuidingCentre g;
+  s = fmin(fmax(s, 0.0), 1.0);          // precondition 0 <= s <= 1; outside values deposit at the bound
   g.s = s;
   double ts = wrap_2pi(th);
   if (ts < 0.0) ts += kTwoPi;           // rounding of the reciprocal multiply
@@ -37,6 +39,8 @@ __device__ __forceinline__ GuidingCentre guiding_centre(const Params& P, double 
   const double e = P.eps * s;
   double sn, cs;
   sincos(ts, &sn, &cs);
+  g.cg = cs;
+  g.sg = sn;
   double two_mu_over_b;
   if (P.theta_map) {
     const double d = fma(-e, cs, 1.0);          // 1 - e cos(theta*)
@@ -80,6 +84,85 @@ __device__ __forceinline__ void larmor_point(const Params& P, const GuidingCentr
   }
 }
 
+// ---- branch-free fp64 building blocks of the per-point geometry.  The library sqrt / division /
+// atan2 carry special-case branches; straight-line code lets the compiler interleave the four
+// Larmor points a producer lane works on (the path is bound by fp64 latency, not by operation count).
+
+// sqrt(x) for normal positive x (<= 1 ulp): MUFU seed (about 20 bits) + two coupled Newton steps
+// + one residual correction.  *half_inv receives 0.5 / sqrt(x).
+__device__ __forceinline__ double sqrt_pos(double x, double* half_inv) {
+  double y;
+  asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
+  double g = x * y, h = 0.5 * y;
+  double r = fma(-g, h, 0.5);
+  g = fma(g, r, g);
+  h = fma(h, r, h);
+  r = fma(-g, h, 0.5);
+  g = fma(g, r, g);
+  h = fma(h, r, h);
+  const double d = fma(-g, g, x);
+  *half_inv = h;
+  return fma(d, h, g);
+}
+
+// a / b for normal b (<= 1 ulp): MUFU seed + two Newton steps + one residual correction
+__device__ __forceinline__ double div_fast(double a, double b) {
+  double y;
+  asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(b));
+  double e = fma(-b, y, 1.0);
+  y = fma(y, e, y);
+  e = fma(-b, y, 1.0);
+  y = fma(y, e, y);
+  const double t = a * y;
+  return fma(fma(-b, t, a), y, t);
+}
+
+// atan(t) for |t| <= 1/4: t * P(t^2), Taylor coefficients (-1)^k / (2k+1) up to k = 12
+// (truncation error <= (1/16)^13 / 27 < 1e-17 relative)
+constexpr double kAtanSmallMax = 0.25;
+__device__ __forceinline__ double atan_small(double t) {
+  const double u = t * t;
+  double p = 1.0 / 25.0;
+  p = fma(p, u, -1.0 / 23.0);
+  p = fma(p, u, 1.0 / 21.0);
+  p = fma(p, u, -1.0 / 19.0);
+  p = fma(p, u, 1.0 / 17.0);
+  p = fma(p, u, -1.0 / 15.0);
+  p = fma(p, u, 1.0 / 13.0);
+  p = fma(p, u, -1.0 / 11.0);
+  p = fma(p, u, 1.0 / 9.0);
+  p = fma(p, u, -1.0 / 7.0);
+  p = fma(p, u, 1.0 / 5.0);
+  p = fma(p, u, -1.0 / 3.0);
+  return fma(t * u, p, t);
+}
+
+// a4 + a5, fast form: Larmor point -> (s_l, theta*_l) with theta*_l = theta*_gc + atan(cross / dot),
+// where (X, Y) = (x + e r, sqrt(1-e^2) z) points along theta*_l (see the header of this file) and
+// (cg, sg) = (cos, sin)(theta*_gc): the ring is small against the minor radius, so the angle between
+// the two is small and a short odd polynomial replaces atan2.  *ok is false when it is not (rings
+// that come near the axis); the caller then takes atan2(Y, X) from (*X, *Y).
+__device__ __forceinline__ void larmor_point_fast(const Params& P, double x0, double z0, double rho,
+                                                  double ts_gc, double cg, double sg, double2 cs_l,
+                                                  double& s_l, double& ts_l, double& X, double& Y,
+                                                  bool& ok) {
+  const double x = fma(rho, cs_l.x, x0);
+  const double z = fma(rho, cs_l.y, z0);
+  const double r2 = fmax(fma(x, x, z * z), 1e-280);
+  double hinv;
+  const double r = sqrt_pos(r2, &hinv);
+  s_l = fmin(r, 1.0);                                   // R11: clamp to the edge
+  const double e = (P.theta_map ? P.eps : 0.0) * s_l;
+  const double q = sqrt_pos(fma(-e, e, 1.0), &hinv);
+  X = fma(e, r, x);
+  Y = q * z;
+  const double dot = fma(X, cg, Y * sg);
+  const double cross = fma(Y, cg, -(X * sg));
+  ok = fabs(cross) <= kAtanSmallMax * dot && dot > 0.0;   // false for NaN
+  const double t = div_fast(cross, fmax(dot, 1e-280));
+  ts_l = ts_gc + atan_small(ok ? t : 0.0);
+}
+
 // Periodic cardinal cubic B-spline weights at cell-unit coordinate x in [0, n]:
 // cell c = floor(x) (may equal n by rounding: wraps), first node c-1.
 __device__ __forceinline__ void cardinal_weights(double t, double w[4]) {
@@ -91,38 +174,26 @@ __device__ __forceinline__ void cardinal_weights(double t, double w[4]) {
   w[3] = t2 * t * (1.0 / 6.0);
 }
 
-__device__ __forceinline__ double open_knot(int i, int n) { return (double)min(max(i - 3, 0), n); }
-
-// Clamped (open knot vector) cubic B-splines, general cell: triangular Cox-de Boor
-// scheme.  Only the two cells at each end differ from the cardinal polynomials.
-static __device__ __noinline__ void clamped_end_weights(double x, int c, int n, double w[4]) {
-  const int span = c + 3;
-  double left[4], right[4];
-  w[0] = 1.0;
+// a6, radial: the 4 weights of bases c..c+3 on radial cell c at in-cell coordinate t.  Cells
+// 2..ns-3 carry the cardinal pieces; the two cells at each end of the clamped (open knot vector)
+// basis differ and come from the host-built table of polynomial pieces (orb_spline_table.cu).
+__device__ __forceinline__ void radial_cell_weights(const Params& P, int c, double t, double w[4]) {
+  if (c >= 2 && c <= P.ns - 3) {
+    cardinal_weights(t, w);
+  } else {
+    const double* tb = P.scoef + (size_t)c * 16;
 #pragma unroll
-  for (int j = 1; j <= 3; ++j) {
-    left[j] = x - open_knot(span + 1 - j, n);
-    right[j] = open_knot(span + j, n) - x;
-    double saved = 0.0;
-#pragma unroll
-    for (int r = 0; r < j; ++r) {
-      const double tmp = w[r] / (right[r + 1] + left[j - r]);
-      w[r] = fma(right[r + 1], tmp, saved);
-      saved = left[j - r] * tmp;
-    }
-    w[j] = saved;
+    for (int a = 0; a < 4; ++a)
+      w[a] = fma(fma(fma(__ldg(tb + a * 4 + 3), t, __ldg(tb + a * 4 + 2)), t, __ldg(tb + a * 4 + 1)),
+                 t, __ldg(tb + a * 4));
   }
 }
 
 // a6, radial: cell i0 (= first basis index) and the 4 weights of bases i0..i0+3.
 __device__ __forceinline__ int radial_weights(const Params& P, double s_l, double w[4]) {
   const double x = s_l * (double)P.ns;
-  int c = min((int)x, P.ns - 1);       // s_l >= 0
-  if (c >= 2 && c <= P.ns - 3) {
-    cardinal_weights(x - (double)c, w);
-  } else {
-    clamped_end_weights(x, c, P.ns, w);
-  }
+  const int c = min(max((int)x, 0), P.ns - 1);
+  radial_cell_weights(P, c, x - (double)c, w);
   return c;
 }
 

@@ -70,6 +70,13 @@ int launch_bin(const Params& P, const Markers& M, const BinScratch& B, bool pres
 int launch_deposit_tile(const Params& P, const Markers& M, const uint32_t* cell_start, double* rho,
                         double* jpar, unsigned long long* d_points, cudaStream_t st);
 
+// v5: one persistent, warp-specialised block per SM (orb_deposit_ws.cu); sms = multiprocessors
+int launch_deposit_ws(const Params& P, const Markers& M, const uint32_t* cell_start, double* rho,
+                      double* jpar, unsigned long long* d_points, int sms, cudaStream_t st);
+
+// ring table (cos, sin)(alpha0 + 2 pi l / N), built on the device (orb_ring.cu)
+int launch_ring_table(double2* ring, double alpha0, cudaStream_t st);
+
 // host: polynomial pieces of the clamped radial cubic B-splines, ns*16 doubles
 void build_radial_table(int ns, std::vector<double>& out);
 

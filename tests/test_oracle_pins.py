@@ -184,6 +184,80 @@ def test_ring_geometry():
     np.testing.assert_allclose(r["x"], np.roll(r0["x"], -1), atol=1e-15)
 
 
+def independent_ring(s, ts, mu, n, *, r0, a, b0, rho_star, alpha0=0.0):
+    """Larmor points by a route that shares nothing with the oracle: theta by root-finding on the
+    quadrature of the straight-field-line relation, B = B0 R0 / R with R = R0 + a s cos(theta) (R1,
+    R2), rho_L = rho* sqrt(2 mu / B) in units of a (R6), ring in the (x, z) plane (R5, R7), theta*
+    of every point by quadrature again (R3) with e_l = (a / R0) s_l.  -> (rho_L, x, z, s_l, ts_l)"""
+    eps = a / r0
+    th = theta_by_root_finding(ts, eps * s)
+    R = r0 + a * s * math.cos(th)
+    B = b0 * r0 / R
+    rho = rho_star * math.sqrt(2 * mu / B)
+    x0, z0 = s * math.cos(th), s * math.sin(th)
+    al = alpha0 + TWO_PI * np.arange(n) / n
+    x, z = x0 + rho * np.cos(al), z0 + rho * np.sin(al)
+    sl = np.minimum(np.hypot(x, z), 1.0)
+    tsl = []
+    for xl, zl, s_l in zip(x, z, sl):
+        thl = math.atan2(zl, xl) % TWO_PI
+        el = eps * s_l
+        v, _ = integrate.quad(lambda t: math.sqrt(1 - el * el) / (1 + el * math.cos(t)), 0, thl,
+                              epsabs=1e-14, epsrel=1e-14)
+        tsl.append(v)
+    return rho, x, z, sl, np.array(tsl)
+
+
+@pytest.mark.parametrize("r0,a,b0", [(1.7, 0.5, 2.5), (3.0, 0.9, 0.4), (1.0, 0.3, 1.0)])
+def test_ring_geometry_nondefault_r0_a_b0(r0, a, b0):
+    """R1, R2, R6 away from the defaults: oracle_larmor_radius and oracle_ring_points against the
+    independent route (a mistake such as eps = a * r0, or a dropped B0, fails here)."""
+    rs = 1 / 15.0
+    g = O.geom(16, 32, 16, r0=r0, a=a, b0=b0, rho_star=rs)
+    rng = np.random.default_rng(5)
+    for n in (4, 7):
+        pol = O.policy_fixed(n, alpha0=0.3)
+        for _ in range(6):
+            s, ts, mu = rng.uniform(0.25, 0.7), rng.uniform(0.1, 6.1), rng.uniform(0.1, 1.5)
+            rho, x, z, sl, tsl = independent_ring(s, ts, mu, n, r0=r0, a=a, b0=b0, rho_star=rs,
+                                                  alpha0=0.3)
+            assert abs(O.larmor_radius(g, s, ts, mu) - rho) < 1e-13
+            r = O.ring_points(g, pol, s, ts, mu)
+            np.testing.assert_allclose(r["x"], x, rtol=0, atol=1e-12)
+            np.testing.assert_allclose(r["z"], z, rtol=0, atol=1e-12)
+            np.testing.assert_allclose(r["s"], sl, rtol=0, atol=1e-12)
+            d = np.abs(r["thetastar"] - tsl)
+            assert np.minimum(d, TWO_PI - d).max() < 1e-11
+
+
+def test_brute_force_nondefault_geometry():
+    """P4 with r0, a, b0, q, rho*, alpha0 all away from their defaults and the Larmor points taken
+    from the independent route, not from the oracle: a node-centric gather with the function
+    definitions of the splines."""
+    ns, nt, nph = 6, 7, 5
+    r0, a, b0, q, rs, alpha0, nl = 1.7, 0.5, 2.5, -1.3, 0.06, 0.37, 4
+    m = small_markers(60, seed=9, s_lo=0.1, s_hi=0.9)
+    g = O.geom(ns, nt, nph, r0=r0, a=a, b0=b0, rho_star=rs, q=q)
+    rho, jp, npts = dep(g, O.policy_fixed(nl, alpha0=alpha0), m)
+    assert npts == 60 * nl
+    T = open_knots(ns)
+    want = np.zeros((ns + 3, nt, nph))
+    wantj = np.zeros_like(want)
+    for p in range(60):
+        _, _, _, sl_, tsl_ = independent_ring(m["s"][p], m["theta"][p], m["mu"][p], nl, r0=r0, a=a,
+                                              b0=b0, rho_star=rs, alpha0=alpha0)
+        lp = np.array([periodic_basis(k, m["phi"][p], nph) for k in range(nph)])
+        for sl, tsl in zip(sl_, tsl_):
+            ls = np.array([cox_de_boor(i, 3, T, sl * ns) for i in range(ns + 3)])
+            lt = np.array([periodic_basis(j, tsl, nt) for j in range(nt)])
+            t3 = ls[:, None, None] * lt[None, :, None] * lp[None, None, :]
+            want += q * m["w"][p] / nl * t3
+            wantj += q * m["w"][p] / nl * m["vpar"][p] * t3
+    scale = np.abs(want).max()
+    assert np.abs(rho - want).max() < 1e-10 * scale
+    assert np.abs(jp - wantj).max() < 1e-10 * np.abs(wantj).max()
+
+
 def test_ring_clamp_and_axis():
     """R11 (ii): points beyond the edge are moved to s = 1; a ring enclosing the axis is legal."""
     g = O.geom(16, 32, 16, rho_star=0.2)

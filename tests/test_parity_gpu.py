@@ -17,7 +17,8 @@ pytestmark = pytest.mark.gpu
 ALGOS = {
     "atomic": B.ORB_DEPOSIT_ALGO_ATOMIC,
     "atomic_nobin": B.ORB_DEPOSIT_ALGO_ATOMIC | B.ORB_DEPOSIT_NO_BIN,
-    "tile": 0,
+    "tile_v4": B.ORB_DEPOSIT_ALGO_TILE_V4,
+    "tile": 0,          # the product path: persistent warp-specialised tile kernel (v5)
 }
 
 
