@@ -748,7 +748,6 @@ __device__ __forceinline__ void consumer(Smem<G, PW, CW>& S, const Params& P,
       const int c_first = lr * kCW + sg * kSegW;
       // node (row lr + a, column sg*kSegW + n), channels 2kk, 2kk+1
       double* pbase = S.tile + ((lr + a) * kNW + sg * kSegW) * kChan + 2 * kk;
-      int idle = 4;   // cells since the last one that had points: >= 4 means all slots are zero
       double c0a = 0.0, c0b = 0.0, c1a = 0.0, c1b = 0.0;
 
       // The batches of a row segment are contiguous in the sorted order: one linear operand
@@ -781,39 +780,29 @@ __device__ __forceinline__ void consumer(Smem<G, PW, CW>& S, const Params& P,
         dmma884(c1a, c1b, a1, bb);                                                    \
       }
 
-#define ORB_RETIRE(U, NCOL)                                                           \
-      if (idle < 4) {                                                                 \
-        double* dst = pbase + (NCOL) * kChan;                                         \
-        if (G == 2 || kk < 2) {                                                       \
-          if ((U) < 2) {                                                              \
-            if (hi == (U)) {                                                          \
-              atomicAdd(dst, c0a);                                                    \
-              atomicAdd(dst + 1, c0b);                                                \
-            }                                                                         \
-          } else {                                                                    \
-            if (hi == (U) - 2) {                                                      \
-              atomicAdd(dst, c1a);                                                    \
-              atomicAdd(dst + 1, c1b);                                                \
-            }                                                                         \
-          }                                                                           \
-        }                                                                             \
-        if ((U) < 2) {                                                                \
-          if (hi == (U)) { c0a = 0.0; c0b = 0.0; }                                    \
-        } else {                                                                      \
-          if (hi == (U) - 2) { c1a = 0.0; c1b = 0.0; }                                \
-        }                                                                             \
-        __syncwarp();   /* the CAS loops diverge; mma.sync.aligned needs the warp whole */ \
+      // Column retire, deferred: stepping past cell U of a group of four finishes one node column
+      // of the window.  Its two accumulators are parked in registers (t0: the column this lane's
+      // first slot held, t1: the second) and all parked columns are added into the shared tile
+      // in one pipelined pass after the walk -- one round of CAS latency per row segment instead
+      // of two per cell.
+#define ORB_PARK(U)                                                                   \
+      if ((U) < 2) {                                                                  \
+        if (hi == (U)) { t0a = c0a; t0b = c0b; c0a = 0.0; c0b = 0.0; }                \
+      } else {                                                                        \
+        if (hi == (U) - 2) { t1a = c1a; t1b = c1b; c1a = 0.0; c1b = 0.0; }            \
       }
 
 #define ORB_CELL(U)                                                                   \
       {                                                                               \
         int nb = (int)(((pk >> 16) + 3u) >> 2);                                       \
         pk = St.cs[c_first + cc + (U) + 1];                                           \
-        idle = nb ? 0 : idle + 1;                                                     \
         for (; nb > 0; --nb) ORB_BATCH                                                \
-        ORB_RETIRE(U, cc + (U))                                                       \
+        ORB_PARK(U)                                                                   \
       }
 
+      // parked columns: pair i holds node columns 4i + hi (first slot) and 4i + hi + 2 (second)
+      double q0a[4], q0b[4], q1a[4], q1b[4];
+      double t0a = 0.0, t0b = 0.0, t1a = 0.0, t1b = 0.0;
       __syncwarp();   // mma.sync.aligned below needs the whole warp converged
 #pragma unroll 1
       for (int cc = 0; cc < kSegW; cc += 4) {
@@ -821,15 +810,63 @@ __device__ __forceinline__ void consumer(Smem<G, PW, CW>& S, const Params& P,
         ORB_CELL(1)
         ORB_CELL(2)
         ORB_CELL(3)
+#pragma unroll
+        for (int i = 0; i < 3; ++i)
+          if (cc == 4 * i) {
+            q0a[i] = t0a; q0b[i] = t0b; q1a[i] = t1a; q1b[i] = t1b;
+          }
       }
-      ++idle;
-      ORB_RETIRE(0, kSegW)
-      ++idle;
-      ORB_RETIRE(1, kSegW + 1)
-      ++idle;
-      ORB_RETIRE(2, kSegW + 2)
+      // the three columns beyond the last cell: 12 + hi (first slot), 14 (second slot, hi = 0)
+      q0a[3] = c0a; q0b[3] = c0b;
+      q1a[3] = hi == 0 ? c1a : 0.0;
+      q1b[3] = hi == 0 ? c1b : 0.0;
+
+      if (G == 2 || kk < 2) {
+        unsigned long long* col0 = reinterpret_cast<unsigned long long*>(pbase + hi * kChan);
+#pragma unroll
+        for (int s2 = 0; s2 < 2; ++s2) {
+          // four columns per pass: loads, adds and CAS of the pass are independent
+          unsigned long long* ad[4];
+          unsigned long long oa[4], ob[4], na[4], nb2[4];
+          double va[4], vb[4];
+          bool live[4];
+#pragma unroll
+          for (int i = 0; i < 4; ++i) {
+            ad[i] = col0 + (4 * i + 2 * s2) * kChan;
+            va[i] = s2 ? q1a[i] : q0a[i];
+            vb[i] = s2 ? q1b[i] : q0b[i];
+            live[i] = va[i] != 0.0 || vb[i] != 0.0;
+          }
+#pragma unroll
+          for (int i = 0; i < 4; ++i)
+            if (live[i]) {
+              const ulonglong2 o = *reinterpret_cast<const ulonglong2*>(ad[i]);
+              oa[i] = o.x;
+              ob[i] = o.y;
+            }
+#pragma unroll
+          for (int i = 0; i < 4; ++i) {
+            na[i] = (unsigned long long)__double_as_longlong(__longlong_as_double((long long)oa[i]) + va[i]);
+            nb2[i] = (unsigned long long)__double_as_longlong(__longlong_as_double((long long)ob[i]) + vb[i]);
+          }
+          unsigned long long ga[4], gb2[4];
+#pragma unroll
+          for (int i = 0; i < 4; ++i)
+            if (live[i]) {
+              ga[i] = atomicCAS(ad[i], oa[i], na[i]);
+              gb2[i] = atomicCAS(ad[i] + 1, ob[i], nb2[i]);
+            }
+#pragma unroll
+          for (int i = 0; i < 4; ++i)
+            if (live[i]) {   // rare: another warp updated the node in between
+              if (ga[i] != oa[i]) atomicAdd(reinterpret_cast<double*>(ad[i]), va[i]);
+              if (gb2[i] != ob[i]) atomicAdd(reinterpret_cast<double*>(ad[i] + 1), vb[i]);
+            }
+        }
+      }
+      __syncwarp();
+#undef ORB_PARK
 #undef ORB_CELL
-#undef ORB_RETIRE
 #undef ORB_BATCH
     }
     __syncwarp();
