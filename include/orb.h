@@ -184,14 +184,30 @@ int orb_deposit_host(orb_grid_t *g, int64_t n, const double *s, const double *th
                      double *rho_host, double *jpar_host, const orb_nl_policy_t *policy,
                      int64_t *n_points, int64_t *h2d_bytes, int64_t *d2h_bytes);
 
+/* Number of kernel launches the library has enqueued on this handle so far
+ * (memsets and copies not counted). */
+int orb_launch_count(const orb_grid_t *g, int64_t *n_launches);
+
+/* ------------------------------------------------------------------------------------------
+ * Harness and diagnostic calls.  NOT part of the product path: nothing above needs them; they
+ * exist so that tests and bench.py can look inside (binned order, per-phase clocks, spline
+ * table) and measure the fp64 roof of the device the bench runs on.  All are synchronous.
+ * ------------------------------------------------------------------------------------------ */
+
 /* Diagnostic: the 16 device counters of the last orb_deposit.  out[0] = Larmor points,
  * out[1] = points deposited directly; out[2..15] = per-phase SM clock sums of the tile kernel
  * (block-thread 0), non-zero only in a library built with -DORB_PHASE_CLOCKS.  Synchronises. */
 int orb_debug_counters(orb_grid_t *g, uint64_t out[16]);
 
-/* Number of kernel launches the library has enqueued on this handle so far
- * (memsets and copies not counted). */
-int orb_launch_count(const orb_grid_t *g, int64_t *n_launches);
+/* Diagnostic: copies the result of the last binning pass to the HOST (bucket sort of
+ * PAPER.md:167; R17, R18).  cell_start_host (ncells + 1 uint32, ncells = ns*ntheta*nphi):
+ * exclusive offsets per guiding-centre cell in key order (k_phi*ns + i_s)*ntheta + j_theta.
+ * *rec_doubles receives the record stride in doubles (8: s, theta*, phi, vpar, mu, w, 0, 0) and
+ * rec_host (n * 8 doubles, may be NULL) the binned records -- or 0 and nothing if the markers
+ * were bound with ORB_MARKERS_SORTED (then the bound order IS the binned order).
+ * ORB_E_STATE if the markers are not binned.  Synchronises the device. */
+int orb_debug_binned(orb_grid_t *g, double *rec_host, uint32_t *cell_start_host,
+                     int32_t *rec_doubles);
 
 /* Host-only diagnostic, no device needed: the polynomial pieces of the clamped (open knot
  * vector) radial cubic B-splines that the tile kernel evaluates (R11).
@@ -204,6 +220,8 @@ int orb_spline_table_radial(int32_t ns, double *out);
  * as TFLOP/s (2 flop per FMA).  The deposition is bound by the fp64 pipe, so this is the roof
  * bench.py reports `roofline_alu` against.  Synchronous; takes a few milliseconds. */
 int orb_probe_dfma(int32_t device, double *tflops);
+
+/* ------------------------------------------------------------------------------------------ */
 
 /* Static text for a status code. */
 const char *orb_strerror(int code);

@@ -23,7 +23,7 @@ ORB_MAX_NL = 32
 # every symbol include/orb.h declares
 SYMBOLS = ("orb_grid_create", "orb_grid_destroy", "orb_grid_shape", "orb_markers_bind",
            "orb_reserve", "orb_markers_bin", "orb_deposit", "orb_grid_zero", "orb_last_points", "orb_last_fallback_points", "orb_deposit_host",
-           "orb_launch_count", "orb_debug_counters", "orb_probe_dfma", "orb_spline_table_radial", "orb_strerror", "orb_last_error", "orb_version")
+           "orb_launch_count", "orb_debug_counters", "orb_debug_binned", "orb_probe_dfma", "orb_spline_table_radial", "orb_strerror", "orb_last_error", "orb_version")
 
 
 class OrbError(RuntimeError):
@@ -70,6 +70,7 @@ def lib():
     L.orb_deposit_host.argtypes = [vp, C.c_int64, dp, dp, dp, dp, dp, dp, dp, dp,
                                    C.POINTER(NlPolicy), i64p, i64p, i64p]
     L.orb_launch_count.argtypes = [vp, i64p]
+    L.orb_debug_binned.argtypes = [vp, dp, dp, C.POINTER(C.c_int32)]
     L.orb_spline_table_radial.argtypes = [C.c_int32, dp]
     L.orb_strerror.argtypes = [C.c_int]
     L.orb_strerror.restype = C.c_char_p
@@ -169,6 +170,17 @@ class Grid:
         out = (C.c_uint64 * 16)()
         _check(lib().orb_debug_counters(self._h, out), self._h)
         return list(out)
+
+    def debug_binned(self, n):
+        """-> (records (n, 8) float64 or None for ORB_MARKERS_SORTED bindings, cell_start uint32)."""
+        import numpy as np
+        ncells = self.desc.ns * self.desc.ntheta * self.desc.nphi
+        cs = np.empty(ncells + 1, dtype=np.uint32)
+        rec = np.empty((n, 8), dtype=np.float64)
+        stride = C.c_int32()
+        _check(lib().orb_debug_binned(self._h, rec.ctypes.data, cs.ctypes.data, C.byref(stride)),
+               self._h)
+        return (rec if stride.value else None), cs
 
     def launch_count(self) -> int:
         v = C.c_int64()

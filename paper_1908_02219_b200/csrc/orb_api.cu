@@ -446,6 +446,23 @@ int orb_debug_counters(orb_grid_t* g, uint64_t out[16]) {
   return ORB_OK;
 }
 
+int orb_debug_binned(orb_grid_t* g, double* rec_host, uint32_t* cell_start_host,
+                     int32_t* rec_doubles) {
+  if (!g || !cell_start_host || !rec_doubles) return ORB_E_INVAL;
+  if (!g->have_bind || !g->binned) return fail(g, ORB_E_STATE, "orb_debug_binned before binning");
+  DeviceGuard dg(g->desc.device);
+  if (!dg.ok) return fail(g, ORB_E_CUDA, "cudaSetDevice");
+  ORB_CUDA(g, cudaDeviceSynchronize());
+  ORB_CUDA(g, cudaMemcpy(cell_start_host, g->bin.cell_start,
+                         (size_t)(g->ncells + 1) * sizeof(uint32_t), cudaMemcpyDeviceToHost));
+  const bool presorted = (g->bind_flags & ORB_MARKERS_SORTED) != 0;
+  *rec_doubles = presorted ? 0 : kRecDoubles;
+  if (!presorted && rec_host && g->bound.n > 0)
+    ORB_CUDA(g, cudaMemcpy(rec_host, g->bin.rec, (size_t)g->bound.n * kRecDoubles * sizeof(double),
+                           cudaMemcpyDeviceToHost));
+  return ORB_OK;
+}
+
 int orb_launch_count(const orb_grid_t* g, int64_t* n) {
   if (!g || !n) return ORB_E_INVAL;
   *n = g->launches;

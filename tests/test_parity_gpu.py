@@ -130,12 +130,150 @@ def test_empty_and_single_marker():
     g.destroy()
 
 
+def _binned(cfg, m, bind_flags=0):
+    """Runs orb_markers_bin alone and reads the binned order back (orb_debug_binned)."""
+    import torch
+    d = to_device(m)
+    g = B.grid_for(cfg)
+    g.markers_bind(d["s"], d["theta"], d["phi"], d["vpar"], d["mu"], d["w"], flags=bind_flags)
+    g.markers_bin(torch.cuda.current_stream().cuda_stream)
+    rec, cs = g.debug_binned(cfg.n_markers)
+    g.destroy()
+    return rec, cs
+
+
 def test_binning_is_a_sort(oracle_results):
-    """a7: binned order has non-decreasing cell keys, is a permutation, and the separately run
-    bin pass + deposit equals deposit alone (P11)."""
+    """a7 (bucket sort of PAPER.md:167; R17, R18): the binned order has non-decreasing cell keys,
+    the per-cell offsets are the histogram's exclusive scan, the records are a permutation of the
+    bound markers (multiset preserved), and bin pass + deposit equals the oracle (P11)."""
     cfg, m, (rho_o, _, _) = get_case("cfg1_small", oracle_results)
+    n = cfg.n_markers
+    rec, cs = _binned(cfg, m)
+    assert rec is not None and rec.shape == (n, 8)
+    key_in = W.cell_key(cfg, m["s"], m["theta"], m["phi"])
+    key_out = W.cell_key(cfg, rec[:, 0], rec[:, 1], rec[:, 2])
+    assert (np.diff(key_out) >= 0).all(), "binned keys must be non-decreasing"
+    ncells = cfg.ns * cfg.ntheta * cfg.nphi
+    hist = np.bincount(key_in, minlength=ncells)
+    assert cs[0] == 0 and cs[-1] == n
+    assert (np.diff(cs.astype(np.int64)) == hist).all(), "cell_start must be the exclusive scan"
+    # every record sits inside its own cell's range
+    assert (cs[key_out] <= np.arange(n)).all() and (np.arange(n) < cs[key_out + 1]).all()
+    # multiset of markers preserved (all six fields, bit for bit) and padding is zero
+    src = np.stack([m[f] for f in W.FIELDS], axis=1)
+    order_in = np.lexsort(src.T[::-1])
+    order_out = np.lexsort(rec[:, :6].T[::-1])
+    assert (src[order_in].view(np.uint64) == rec[order_out, :6].view(np.uint64)).all()
+    assert (rec[:, 6:] == 0).all()
     rho_a, _, _ = run_gpu(cfg, m, bin_first=True)
     assert_parity(rho_a, rho_o)
+
+
+def test_binning_of_presorted_markers_locates_cells(oracle_results):
+    """ORB_MARKERS_SORTED: no records are written; cell_start alone must delimit the cells."""
+    cfg, m, _ = get_case("cfg4s_small", oracle_results)
+    rec, cs = _binned(cfg, m, bind_flags=B.ORB_MARKERS_SORTED)
+    assert rec is None
+    key = W.cell_key(cfg, m["s"], m["theta"], m["phi"])
+    assert (np.diff(key) >= 0).all()
+    hist = np.bincount(key, minlength=cfg.ns * cfg.ntheta * cfg.nphi)
+    assert (np.diff(cs.astype(np.int64)) == hist).all()
+
+
+def test_sorted_flag_on_unsorted_markers_stays_correct(oracle_results):
+    """ORB_MARKERS_SORTED is a hint (include/orb.h): bound to markers that are NOT sorted the
+    result must still be the oracle's (sorted == unsorted)."""
+    for name in ("cfg3_small", "cfg4_small"):
+        cfg, m, (rho_o, jpar_o, npts_o) = get_case(name, oracle_results)
+        for algo in ("tile", "tile_v4"):
+            rho, jpar, npts = run_gpu(cfg, m, flags=ALGOS[algo], bind_flags=B.ORB_MARKERS_SORTED)
+            assert npts == npts_o
+            assert_parity(rho, rho_o, "%s/%s rho" % (name, algo))
+            assert_parity(jpar, jpar_o, "%s/%s jpar" % (name, algo))
+
+
+@pytest.mark.parametrize("adaptive", [False, True])
+def test_angles_outside_0_2pi_and_radial_bounds(adaptive):
+    """include/orb.h: theta*, phi are 'any finite angle' (R13 wrap) and s in [0, 1] INCLUSIVE.
+    theta*, phi in [-7 pi, 9 pi]; a share of the markers has s exactly 0 and exactly 1, angles
+    exactly 0, 2 pi, -2 pi and on cell boundaries."""
+    cfg = small("cfg0", 60_013, current=True, s_lo=0.0, s_hi=1.0, adaptive=adaptive,
+                n_max=16 if adaptive else 4, rho_star=1 / 60.0)
+    m = W.generate(cfg)
+    n = cfg.n_markers
+    turns = (np.arange(n) % 8) - 4                         # -4 .. 3 full turns
+    m["theta"] = m["theta"] + W.TWO_PI * turns + (np.arange(n) % 2) * np.pi   # [-8pi, 9pi)
+    m["theta"] = np.clip(m["theta"], -7 * np.pi, 9 * np.pi)
+    m["phi"] = m["phi"] + W.TWO_PI * ((np.arange(n) // 8) % 8 - 3.5)          # [-7pi, 9pi)
+    m["s"][0:n:17] = 0.0
+    m["s"][1:n:17] = 1.0
+    m["theta"][2:n:17] = 0.0
+    m["theta"][3:n:17] = W.TWO_PI
+    m["theta"][4:n:17] = -W.TWO_PI
+    m["phi"][5:n:17] = 0.0
+    m["phi"][6:n:17] = W.TWO_PI
+    m["phi"][7:n:17] = 3 * W.TWO_PI / cfg.nphi             # on a cell boundary
+    m["theta"][8:n:17] = -5 * W.TWO_PI / cfg.ntheta
+    assert m["theta"].min() < -6 * np.pi and m["theta"].max() > 8 * np.pi
+    assert m["phi"].min() < -6 * np.pi and m["phi"].max() > 8 * np.pi
+    rho_o, jpar_o, npts_o = run_oracle(cfg, m)
+    for algo, flags in ALGOS.items():
+        rho, jpar, npts = run_gpu(cfg, m, flags=flags)
+        assert npts == npts_o
+        assert_parity(rho, rho_o, "wrapped/%s rho" % algo)
+        assert_parity(jpar, jpar_o, "wrapped/%s jpar" % algo)
+
+
+def test_radial_coordinate_outside_0_1_deposits_at_the_bound():
+    """include/orb.h: 's outside [0,1] is treated as the nearest bound' (R11) -- s = -0.2 and 1.2
+    must give exactly what s = 0 and s = 1 give (and never write out of bounds)."""
+    cfg = small("cfg0", 20_011, current=True, s_lo=0.0, s_hi=1.0)
+    m = W.generate(cfg)
+    n = cfg.n_markers
+    bad = dict(m)
+    bad["s"] = m["s"].copy()
+    bad["s"][0:n:5] = -0.2
+    bad["s"][1:n:5] = 1.2
+    bad["s"][2:n:5] = -1e-300
+    ref = dict(m)
+    ref["s"] = np.clip(bad["s"], 0.0, 1.0)
+    rho_o, jpar_o, npts_o = run_oracle(cfg, ref)
+    for algo, flags in ALGOS.items():
+        rho, jpar, npts = run_gpu(cfg, bad, flags=flags)
+        assert npts == npts_o
+        assert_parity(rho, rho_o, "clamped s/%s rho" % algo)
+        assert_parity(jpar, jpar_o, "clamped s/%s jpar" % algo)
+
+
+def test_cuda_graph_capture_of_bin_zero_deposit(oracle_results):
+    """no host synchronisation and no allocation inside orb_markers_bin /
+    orb_grid_zero / orb_deposit -- the three calls are captured into ONE CUDA graph (capture
+    fails on any synchronising call), replayed 3 times, and the grids match the oracle."""
+    import torch
+    for name in ("cfg3_small", "cfg4_small"):
+        cfg, m, (rho_o, jpar_o, npts_o) = get_case(name, oracle_results)
+        d = to_device(m)
+        g = B.grid_for(cfg)
+        rho = torch.full(g.shape(), 3.0, dtype=torch.float64, device="cuda")
+        jpar = torch.full(g.shape(), -2.0, dtype=torch.float64, device="cuda")
+        pol = B.policy_for(cfg)
+        g.markers_bind(d["s"], d["theta"], d["phi"], d["vpar"], d["mu"], d["w"])
+        torch.cuda.synchronize()
+        graph = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(graph):
+            st = torch.cuda.current_stream().cuda_stream
+            g.markers_bin(st)
+            g.grid_zero(rho, jpar, st)
+            g.deposit(rho, jpar, pol, st)
+        for _ in range(3):
+            rho.fill_(9.0)
+            graph.replay()
+        torch.cuda.synchronize()
+        assert g.last_points() == npts_o
+        assert_parity(rho.cpu().numpy(), rho_o, name + " graph rho")
+        assert_parity(jpar.cpu().numpy(), jpar_o, name + " graph jpar")
+        del graph
+        g.destroy()
 
 
 def test_error_codes():
