@@ -70,6 +70,9 @@ def lib():
         L.oracle_deposit.restype = C.c_int64
         L.oracle_deposit.argtypes = [C.POINTER(Geom), C.POINTER(Policy), C.c_int64,
                                      dp, dp, dp, dp, dp, dp, dp, dp]
+        L.oracle_gather.restype = C.c_int64
+        L.oracle_gather.argtypes = [C.POINTER(Geom), C.POINTER(Policy), C.c_int64,
+                                    dp, dp, dp, dp, dp, dp]
         L.oracle_nl_histogram.restype = C.c_int64
         L.oracle_nl_histogram.argtypes = [C.POINTER(Geom), C.POINTER(Policy), C.c_int64,
                                           dp, dp, dp, C.POINTER(C.c_int64)]
@@ -204,6 +207,33 @@ def deposit_ranges(g: Geom, pol: Policy, s, thetastar, phi, vpar, mu, w, *, curr
             jpar += j
         npts += k
     return rho, jpar, npts, workers
+
+
+def gather(g: Geom, pol: Policy, s, thetastar, phi, mu, field, *, workers=1):
+    """Get fields + gyroaverage (oracle_gather): field (ns+3, ntheta, nphi) -> out[n].
+    Markers are independent, so ``workers`` > 1 only splits the marker range over threads and
+    gives bit-identical results.  Returns (out, n_points)."""
+    s, thetastar, phi, mu = map(_f64, (s, thetastar, phi, mu))
+    field = _f64(field)
+    assert field.shape == grid_shape(g), (field.shape, grid_shape(g))
+    n = s.shape[0]
+    out = np.empty(n)
+    L = lib()
+
+    def run(a, b):
+        r = L.oracle_gather(C.byref(g), C.byref(pol), b - a, _dp(s[a:b]), _dp(thetastar[a:b]),
+                            _dp(phi[a:b]), _dp(mu[a:b]), _dp(field), _dp(out[a:b]))
+        if r < 0:
+            raise ValueError("oracle_gather: N_L > %d" % MAX_NL)
+        return int(r)
+
+    workers = max(1, min(workers or (os.cpu_count() or 1), (n + 4095) // 4096 or 1))
+    if workers == 1:
+        return out, run(0, n)
+    bounds = np.linspace(0, n, workers + 1).astype(np.int64)
+    with ThreadPoolExecutor(workers) as ex:
+        npts = sum(ex.map(lambda i: run(int(bounds[i]), int(bounds[i + 1])), range(workers)))
+    return out, npts
 
 
 def nl_histogram(g: Geom, pol: Policy, s, thetastar, mu):

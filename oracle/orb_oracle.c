@@ -252,3 +252,59 @@ int64_t oracle_nl_histogram(const oracle_geom_t *g, const oracle_policy_t *pol, 
   }
   return npts;
 }
+
+/* ------------------------------------------------------------------------------------------
+ * NEXT-1: 'get fields' + 'gyroaverage' -- the transpose of the deposition.
+ *
+ *   out[p] = (1 / N_L(p)) sum_l  sum_{i,j,k} field[i,j,k] Ls_i(s_pl) Lt_j(ts_pl) Lp_k(phi_p)
+ *
+ *   - stage (3) of the PIC step: "the interpolation of the field at particle positions"
+ *     (PAPER.md:71); with the Larmor ring data it splits into 'get fields' at the Larmor
+ *     points and 'gyroaveraging' back to the guiding centre;
+ *   - the field is the finite-element cubic B-spline expansion on the same grid as the
+ *     deposited arrays, same layout (R14);
+ *   - same ring, same points, same splines as oracle_deposit (O1-O6).
+ * Reading R20 (the paper prints no formula): the value at a Larmor point is the spline
+ * expansion evaluated there; the gyro-average is the arithmetic mean over the marker's N_L
+ * points -- the discrete gyro-average whose weights 1/N_L the deposition uses, so that
+ *   sum_n rho[n] field[n] = q sum_p w_p out[p]          (adjointness; pinned)
+ * One field per call (several fields = several calls).  Field gradients are not formed here.
+ * Marker order p = 0..n-1, then l, then the 4x4x4 nodes.  Returns sum_p N_L(p) or -1.
+ * Pins (tests/test_oracle_pins.py): adjointness with oracle_deposit, constant field -> 1,
+ * Greville (linear-in-s) field -> mean of s_pl, dense tensor-product evaluation with scipy
+ * BSpline / periodised beta^3 at the ring points for N_L = 1, 4, 8, linearity in the field.
+ */
+int64_t oracle_gather(const oracle_geom_t *g, const oracle_policy_t *pol, int64_t n,
+                      const double *s, const double *thetastar, const double *phi,
+                      const double *mu, const double *field, double *out) {
+  int64_t npts = 0;
+  double sl[ORACLE_MAX_NL], tsl[ORACLE_MAX_NL];
+  for (int64_t p = 0; p < n; ++p) {
+    {
+      double rl = oracle_larmor_radius(g, s[p], thetastar[p], mu[p]);
+      if (oracle_nl(pol, rl) > ORACLE_MAX_NL) return -1;
+    }
+    int32_t N = oracle_ring_points(g, pol, s[p], thetastar[p], mu[p], sl, tsl, NULL, NULL);
+    int32_t k0;
+    double wphi[4];
+    oracle_periodic_cubic(phi[p], g->nphi, &k0, wphi);
+    double acc = 0.0;
+    for (int32_t l = 0; l < N; ++l) {
+      int32_t i0, j0;
+      double ws[4], wt[4];
+      oracle_clamped_cubic(sl[l], g->ns, &i0, ws);
+      oracle_periodic_cubic(tsl[l], g->ntheta, &j0, wt);
+      for (int a = 0; a < 4; ++a)
+        for (int b = 0; b < 4; ++b)
+          for (int d = 0; d < 4; ++d) {
+            int64_t node = ((int64_t)(i0 + a) * g->ntheta + oracle_mod(j0 + b, g->ntheta)) *
+                               (int64_t)g->nphi +
+                           oracle_mod(k0 + d, g->nphi);
+            acc += ws[a] * wt[b] * wphi[d] * field[node];
+          }
+    }
+    out[p] = acc / (double)N;
+    npts += N;
+  }
+  return npts;
+}

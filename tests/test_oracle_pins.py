@@ -493,3 +493,98 @@ def test_cfg0_regression_golden():
     assert abs(np.abs(rho).max() - want["max_abs"]) < 1e-16
     for (i, j, k), v in zip(want["nodes"], want["values"]):
         assert abs(rho[i, j, k] - v) < 1e-16
+
+
+# ------------------------------------------- NEXT-1: get fields + gyroaverage (oracle_gather) ---
+
+def gat(g, pol, m, field, n=None):
+    n = n or len(m["s"])
+    return O.gather(g, pol, m["s"][:n], m["theta"][:n], m["phi"][:n], m["mu"][:n], field)
+
+
+@pytest.mark.parametrize("policy", ["fixed1", "fixed4", "fixed7", "adaptive"])
+def test_gather_is_the_adjoint_of_deposit(policy):
+    """G1: <deposit(w), F> = q sum_p w_p gather(F)_p for any field F --
+    ties every index, weight and 1/N_L of oracle_gather to the (pinned) oracle_deposit, markers in
+    the radial end cells and rings clamped at s = 1 included."""
+    m = small_markers(3000, seed=11, s_lo=0.0, s_hi=1.0)
+    g = O.geom(12, 9, 7, r0=1.4, a=0.45, b0=1.8, rho_star=0.06, q=-1.7)
+    pol = {"fixed1": O.policy_fixed(1), "fixed4": O.policy_fixed(4), "fixed7": O.policy_fixed(7, 0.3),
+           "adaptive": O.policy_adaptive(4, 16, 0.06)}[policy]
+    rng = np.random.default_rng(5)
+    F = rng.standard_normal(O.grid_shape(g))
+    rho, _, npts = dep(g, pol, m, current=False)
+    out, npts_g = gat(g, pol, m, F)
+    assert npts_g == npts
+    lhs = float((rho * F).sum())
+    rhs = float(g.q * (m["w"] * out).sum())
+    scale = abs(g.q) * np.abs(m["w"]).sum() * np.abs(F).max()
+    assert abs(lhs - rhs) < 1e-13 * scale
+
+
+def test_gather_constant_and_greville_fields():
+    """G2: partition of unity -- a constant field is returned exactly for every marker (also
+    those whose ring is clamped at s = 1 or encloses the axis).  G3: cubic splines reproduce
+    linear functions: with F[i,j,k] = Greville abscissa xi_i the gather returns the mean of
+    s_pl over the ring (ring_points is pinned by P6)."""
+    ns = 10
+    m = small_markers(1500, seed=3, s_lo=0.0, s_hi=1.0)
+    g = O.geom(ns, 12, 6, rho_star=0.09)
+    for pol in (O.policy_fixed(1), O.policy_fixed(4), O.policy_adaptive(4, 32, 0.09)):
+        out, _ = gat(g, pol, m, np.full(O.grid_shape(g), 2.5))
+        np.testing.assert_allclose(out, 2.5, rtol=0, atol=1e-14)
+        T = open_knots(ns)
+        xi = np.array([(T[i + 1] + T[i + 2] + T[i + 3]) / (3 * ns) for i in range(ns + 3)])
+        F = np.broadcast_to(xi[:, None, None], O.grid_shape(g)).copy()
+        out, _ = gat(g, pol, m, F)
+        want = np.array([O.ring_points(g, pol, m["s"][p], m["theta"][p], m["mu"][p])["s"].mean()
+                         for p in range(1500)])
+        np.testing.assert_allclose(out, want, rtol=0, atol=2e-15)
+
+
+@pytest.mark.parametrize("nl", [1, 4, 8])
+def test_gather_dense_tensor_product_evaluation(nl):
+    """G4: out[p] = mean_l sum_ijk F[ijk] Ls_i(s_pl) Lt_j(ts_pl) Lp_k(phi_p) with the basis
+    FUNCTIONS evaluated densely -- scipy BSpline on the open knot vector in s, the periodised
+    beta^3 definition in theta*, phi -- no index logic shared with the oracle.  For N_L = 1 this
+    is plain tensor-product spline interpolation at (s, theta*, phi)."""
+    ns, nt, nph = 6, 5, 7
+    m = small_markers(150, seed=9, s_lo=0.0, s_hi=1.0)
+    g = O.geom(ns, nt, nph, rho_star=0.08)
+    pol = O.policy_fixed(nl)
+    rng = np.random.default_rng(1)
+    F = rng.standard_normal((ns + 3, nt, nph))
+    T = open_knots(ns)
+    basis = [interpolate.BSpline(T, np.eye(ns + 3)[i], 3, extrapolate=False) for i in range(ns + 3)]
+    out, npts = gat(g, pol, m, F)
+    assert npts == 150 * nl
+    want = np.zeros(150)
+    for p in range(150):
+        r = O.ring_points(g, pol, m["s"][p], m["theta"][p], m["mu"][p])
+        lp = np.array([periodic_basis(k, m["phi"][p], nph) for k in range(nph)])
+        for sl, tsl in zip(r["s"], r["thetastar"]):
+            x = min(sl * ns, ns * (1 - 1e-16))
+            ls = np.nan_to_num(np.array([float(b(x)) for b in basis]))
+            lt = np.array([periodic_basis(j, tsl, nt) for j in range(nt)])
+            want[p] += np.einsum("i,j,k,ijk->", ls, lt, lp, F) / nl
+    np.testing.assert_allclose(out, want, rtol=0, atol=2e-14)
+
+
+def test_gather_linearity_rotation_and_threads():
+    """Linear in the field; rotating field and markers by one phi cell leaves the result
+    unchanged (wrap direction, cf. P9); marker ranges on threads are bit-identical."""
+    m = small_markers(5000, seed=2)
+    g = O.geom(16, 32, 16, rho_star=0.03)
+    pol = O.policy_fixed(4)
+    rng = np.random.default_rng(0)
+    F1, F2 = rng.standard_normal((2,) + O.grid_shape(g))
+    o1, _ = gat(g, pol, m, F1)
+    o2, _ = gat(g, pol, m, F2)
+    o12, _ = gat(g, pol, m, 2.0 * F1 - 3.0 * F2)
+    np.testing.assert_allclose(o12, 2.0 * o1 - 3.0 * o2, rtol=0, atol=1e-14)
+    m2 = dict(m)
+    m2["phi"] = m["phi"] + TWO_PI / 16
+    o1r, _ = gat(g, pol, m2, np.roll(F1, 1, axis=2))
+    np.testing.assert_allclose(o1r, o1, rtol=0, atol=1e-13)
+    ot, npts = O.gather(g, pol, m["s"], m["theta"], m["phi"], m["mu"], F1, workers=3)
+    assert npts == 20000 and (ot == o1).all()
