@@ -52,6 +52,7 @@ extern "C" {
 
 #define ORB_VERSION 100
 #define ORB_MAX_NL 32 /* largest number of Larmor points per marker */
+#define ORB_MAX_FIELDS 8 /* fields per orb_gather call */
 
 typedef enum {
   ORB_OK = 0,
@@ -154,6 +155,27 @@ int orb_markers_bin(orb_grid_t *g, void *stream);
 int orb_deposit(orb_grid_t *g, double *rho, double *jpar, const orb_nl_policy_t *policy,
                 void *stream);
 
+/* Get fields + gyroaverage -- the transpose of orb_deposit (stage 3 of the PIC step, "the
+ * interpolation of the field at particle positions"; with the Larmor ring data it
+ * is 'get fields' at the Larmor points followed by 'gyroaveraging' back to the guiding centre,
+ * PAPER.md:73, 89; the paper's largest GPU win).  For every bound marker p and
+ * field f (reading R20 of DESIGN.md: the paper prints no formula):
+ *
+ *   out[f][p] = (1 / N_L(p)) sum_l sum_{i,j,k} fields[f][i,j,k] Ls_i(s_pl) Lt_j(ts_pl) Lp_k(phi_p)
+ *
+ * with the ring, the map and the cubic B-splines of orb_deposit, so that for any field F
+ *   sum_nodes rho[n] F[n] = q sum_p w_p out[p]      (adjointness; rho from orb_deposit).
+ * fields / out: HOST arrays of n_fields (1..ORB_MAX_FIELDS) DEVICE pointers; fields[f] has
+ * orb_grid_shape doubles (layout of rho, 16-byte aligned, only read); out[f] has n doubles and is
+ * written in BOUND marker order whatever the binning did (owned by the caller; the pointer
+ * arrays themselves are read during the call only).  The marker weights and vpar are not used.
+ * Asynchronous on `stream`; bins first if the markers are not binned yet (never allocates);
+ * ORB_DEPOSIT_NO_BIN or ORB_DEPOSIT_ALGO_ATOMIC in policy->flags select the one-thread-per-marker
+ * kernel that reads the grid directly, in bound order.  orb_last_points / orb_last_fallback_points
+ * then refer to this call.  Field gradients are not formed. */
+int orb_gather(orb_grid_t *g, int32_t n_fields, const double *const *fields, double *const *out,
+               const orb_nl_policy_t *policy, void *stream);
+
 /* Zeroes rho and, if not NULL, jpar (DEVICE arrays of orb_grid_shape doubles) on `stream`
  * (two cudaMemsetAsync; no kernel).  Equivalent to ORB_DEPOSIT_ZERO_FIRST, offered as a call of
  * its own so that a harness can time the deposit kernels apart from the zeroing. */
@@ -202,7 +224,8 @@ int orb_debug_counters(orb_grid_t *g, uint64_t out[16]);
 /* Diagnostic: copies the result of the last binning pass to the HOST (bucket sort of
  * PAPER.md:167; R17, R18).  cell_start_host (ncells + 1 uint32, ncells = ns*ntheta*nphi):
  * exclusive offsets per guiding-centre cell in key order (k_phi*ns + i_s)*ntheta + j_theta.
- * *rec_doubles receives the record stride in doubles (8: s, theta*, phi, vpar, mu, w, 0, 0) and
+ * *rec_doubles receives the record stride in doubles (8: s, theta*, phi, vpar, mu, w, the
+ * marker's index in bound order as a 64-bit integer bit pattern, 0) and
  * rec_host (n * 8 doubles, may be NULL) the binned records -- or 0 and nothing if the markers
  * were bound with ORB_MARKERS_SORTED (then the bound order IS the binned order).
  * ORB_E_STATE if the markers are not binned.  Synchronises the device. */

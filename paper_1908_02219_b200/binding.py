@@ -19,10 +19,11 @@ ORB_DEPOSIT_ALGO_ATOMIC = 0x4
 ORB_DEPOSIT_ALGO_TILE_V4 = 0x8
 ORB_MARKERS_SORTED = 0x1
 ORB_MAX_NL = 32
+ORB_MAX_FIELDS = 8
 
 # every symbol include/orb.h declares
 SYMBOLS = ("orb_grid_create", "orb_grid_destroy", "orb_grid_shape", "orb_markers_bind",
-           "orb_reserve", "orb_markers_bin", "orb_deposit", "orb_grid_zero", "orb_last_points", "orb_last_fallback_points", "orb_deposit_host",
+           "orb_reserve", "orb_markers_bin", "orb_deposit", "orb_gather", "orb_grid_zero", "orb_last_points", "orb_last_fallback_points", "orb_deposit_host",
            "orb_launch_count", "orb_debug_counters", "orb_debug_binned", "orb_probe_dfma", "orb_spline_table_radial", "orb_strerror", "orb_last_error", "orb_version")
 
 
@@ -64,6 +65,8 @@ def lib():
     L.orb_reserve.argtypes = [vp, C.c_int64]
     L.orb_markers_bin.argtypes = [vp, vp]
     L.orb_deposit.argtypes = [vp, dp, dp, C.POINTER(NlPolicy), vp]
+    L.orb_gather.argtypes = [vp, C.c_int32, C.POINTER(C.c_void_p), C.POINTER(C.c_void_p),
+                             C.POINTER(NlPolicy), vp]
     L.orb_grid_zero.argtypes = [vp, dp, dp, vp]
     L.orb_last_points.argtypes = [vp, i64p]
     L.orb_last_fallback_points.argtypes = [vp, i64p]
@@ -152,6 +155,13 @@ class Grid:
 
     def deposit(self, rho, jpar, pol: NlPolicy, stream=None):
         _check(lib().orb_deposit(self._h, _ptr(rho), _ptr(jpar), C.byref(pol), stream), self._h)
+
+    def gather(self, fields, out, pol: NlPolicy, stream=None):
+        """fields: sequence of device grids; out: sequence of device arrays of n doubles."""
+        nf = len(fields)
+        fa = (C.c_void_p * nf)(*[_ptr(f) for f in fields])
+        oa = (C.c_void_p * nf)(*[_ptr(o) for o in out])
+        _check(lib().orb_gather(self._h, nf, fa, oa, C.byref(pol), stream), self._h)
 
     def grid_zero(self, rho, jpar, stream=None):
         _check(lib().orb_grid_zero(self._h, _ptr(rho), _ptr(jpar), stream), self._h)

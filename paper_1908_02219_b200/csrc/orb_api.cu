@@ -406,6 +406,48 @@ int orb_deposit(orb_grid_t* g, double* rho, double* jpar, const orb_nl_policy_t*
   return ORB_OK;
 }
 
+int orb_gather(orb_grid_t* g, int32_t n_fields, const double* const* fields, double* const* out,
+               const orb_nl_policy_t* pol, void* stream) {
+  if (!g) return ORB_E_INVAL;
+  if (n_fields < 1 || n_fields > ORB_MAX_FIELDS) return fail(g, ORB_E_INVAL, "n_fields out of [1, ORB_MAX_FIELDS]");
+  if (!fields || !out) return fail(g, ORB_E_INVAL, "fields / out is NULL");
+  int rc = check_policy(g, pol);
+  if (rc != ORB_OK) return rc;
+  if (!g->have_bind) return fail(g, ORB_E_STATE, "orb_gather before orb_markers_bind");
+  for (int f = 0; f < n_fields; ++f) {
+    if (!fields[f] || (!out[f] && g->bound.n > 0)) return fail(g, ORB_E_INVAL, "NULL field / out pointer");
+    if (!aligned16(fields[f])) return fail(g, ORB_E_INVAL, "fields must be 16-byte aligned");
+  }
+  DeviceGuard dg(g->desc.device);
+  if (!dg.ok) return fail(g, ORB_E_CUDA, "cudaSetDevice");
+  cudaStream_t st = static_cast<cudaStream_t>(stream);
+  rc = upload_ring(g, pol->alpha0, st);
+  if (rc != ORB_OK) return rc;
+  const bool direct = (pol->flags & (ORB_DEPOSIT_NO_BIN | ORB_DEPOSIT_ALGO_ATOMIC)) != 0;
+  if (!direct && !g->binned) {
+    rc = do_bin(g, st);
+    if (rc != ORB_OK) return rc;
+  }
+  ORB_CUDA(g, cudaMemsetAsync(g->d_points, 0, kCounters * sizeof(unsigned long long), st));
+  Params P = make_params(g, pol);
+  Markers M = g->bound;
+  const bool presorted = (g->bind_flags & ORB_MARKERS_SORTED) != 0;
+  if (!direct && !presorted) M.rec = g->bin.rec;
+  int l = launch_gather(P, M, g->bin.cell_start, n_fields, fields, out, g->d_points, !direct, st);
+  if (l < 0) return fail(g, ORB_E_CUDA, "gather launch", cudaGetLastError());
+  g->launches += l;
+  ORB_CUDA(g, cudaGetLastError());
+  cudaStreamCaptureStatus cap = cudaStreamCaptureStatusNone;
+  if (cudaStreamIsCapturing(st, &cap) != cudaSuccess) cudaGetLastError();
+  if (cap == cudaStreamCaptureStatusNone) {
+    ORB_CUDA(g, cudaEventRecord(g->dep_event, st));
+    g->dep_event_valid = true;
+  } else {
+    g->dep_event_valid = false;
+  }
+  return ORB_OK;
+}
+
 int orb_grid_zero(orb_grid_t* g, double* rho, double* jpar, void* stream) {
   if (!g) return ORB_E_INVAL;
   if (!rho) return fail(g, ORB_E_INVAL, "rho is NULL");

@@ -7,7 +7,8 @@
 //   1. count:   rank[p] = atomicAdd(count[key(p)], 1)       (integer atomics in L2)
 //   2. scan:    cell_start = exclusive prefix sum of count   (3 small kernels)
 //   3. scatter: record(cell_start[key(p)] + rank[p]) = marker p, as one 64-byte
-//               record {s, theta*, phi, vpar, mu, w, 0, 0} (four 16-byte stores) so
+//               record {s, theta*, phi, vpar, mu, w, index in bound order, 0} (two 32-byte
+//               stores) so
 //               that a random-order input costs 2 whole sectors per marker, not 6
 //               partial ones.
 // The order inside a cell is whatever the atomics gave (any order is correct, R18).
@@ -135,8 +136,10 @@ k_bin_scatter(const Params P, const Markers M, const uint32_t* __restrict__ cell
   const double mu = __ldg(M.mu + p), w = __ldg(M.w + p);
   asm volatile("st.global.v4.f64 [%0], {%1, %2, %3, %4};" ::"l"(out), "d"(s), "d"(th), "d"(ph), "d"(vp)
                : "memory");
-  asm volatile("st.global.v4.f64 [%0], {%1, %2, %3, %4};" ::"l"(out + 4), "d"(mu), "d"(w), "d"(0.0),
-               "d"(0.0)
+  // slot 6: the marker's index in bound order (bit pattern), for results that go back to the
+  // caller's order (orb_gather)
+  asm volatile("st.global.v4.f64 [%0], {%1, %2, %3, %4};" ::"l"(out + 4), "d"(mu), "d"(w),
+               "d"(__longlong_as_double((long long)p)), "d"(0.0)
                : "memory");
 }
 

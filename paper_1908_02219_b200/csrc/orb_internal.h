@@ -12,7 +12,8 @@ namespace orb {
 
 constexpr double kTwoPi = 6.283185307179586476925286766559;
 constexpr int kCounters = 16;    // device counters: [0] Larmor points, [1] direct-path points, [2..] debug
-// binned marker record: s, theta*, phi, vpar, mu, w + 2 doubles of padding.  64 bytes = two whole
+// binned marker record: s, theta*, phi, vpar, mu, w, the marker's index in bound order (an
+// integer bit pattern) + 1 double of padding.  64 bytes = two whole
 // 32-byte sectors, so the random-order scatter of the counting sort never leaves a partially
 // written sector for DRAM to read back (48-byte records cost 6.6 GB of fill reads on cfg3).
 constexpr int kRecDoubles = 8;
@@ -73,6 +74,11 @@ int launch_deposit_tile(const Params& P, const Markers& M, const uint32_t* cell_
 // v5: one persistent, warp-specialised block per SM (orb_deposit_ws.cu); sms = multiprocessors
 int launch_deposit_ws(const Params& P, const Markers& M, const uint32_t* cell_start, double* rho,
                       double* jpar, unsigned long long* d_points, int sms, cudaStream_t st);
+
+// get fields + gyroaverage (orb_gather.cu); fields / out: host arrays of n_fields device pointers
+int launch_gather(const Params& P, const Markers& M, const uint32_t* cell_start, int n_fields,
+                  const double* const* fields, double* const* out, unsigned long long* d_points,
+                  bool tiled, cudaStream_t st);
 
 // ring table (cos, sin)(alpha0 + 2 pi l / N), built on the device (orb_ring.cu)
 int launch_ring_table(double2* ring, double alpha0, cudaStream_t st);

@@ -177,3 +177,42 @@ def test_deposit_host_sliced_pipeline():
         assert rel_err(rho, rho_o) <= TOL
         assert rel_err(jpar, jpar_o) <= TOL
     g.destroy()
+
+
+@pytest.mark.parametrize("name", ["cfg3", "cfg4"])
+def test_gather_full_size_sampled_markers(name):
+    """orb_gather (NEXT-1) at full size in the configuration bench.py times (bind -> bin ->
+    gather of 2 fields): the GPU computes every marker; a marker's result depends on that marker
+    alone, so the oracle computes a seeded sample of 2^21 markers one by one and those outputs
+    are compared element by element.  Property at full size: a constant field returns 1 for
+    every marker (partition of unity), which also proves every marker was written."""
+    import torch
+    if name == "cfg4" and (_host_mem_gb() < 60.0 or torch.cuda.mem_get_info()[1] < 60e9):
+        pytest.skip("cfg4 needs ~40 GB of host and ~25 GB of device memory")
+    cfg = W.CONFIGS[name]
+    m = W.generate(cfg)
+    n = cfg.n_markers
+    rng = np.random.default_rng(17)
+    shape = (cfg.ns + 3, cfg.ntheta, cfg.nphi)
+    fields = [rng.standard_normal(shape), np.ones(shape)]
+    d = {f: torch.from_numpy(m[f]).cuda() for f in W.FIELDS if f != "vpar"}
+    fd = [torch.from_numpy(f).cuda() for f in fields]
+    out = [torch.full((n,), np.nan, dtype=torch.float64, device="cuda") for _ in fields]
+    g = B.grid_for(cfg)
+    st = torch.cuda.current_stream().cuda_stream
+    g.markers_bind(d["s"], d["theta"], d["phi"], None, d["mu"], d["w"])
+    g.markers_bin(st)
+    g.gather(fd, out, B.policy_for(cfg), st)
+    torch.cuda.synchronize()
+    npts, fallback = g.last_points(), g.last_fallback_points()
+    g.destroy()
+    assert fallback < 0.01 * npts
+    ones = out[1].cpu().numpy()
+    assert np.abs(ones - 1.0).max() <= 1e-13
+    idx = np.sort(rng.choice(n, size=1 << 21, replace=False))
+    want, _ = O.gather(oracle_geom(cfg), oracle_policy(cfg), m["s"][idx], m["theta"][idx],
+                       m["phi"][idx], m["mu"][idx], fields[0], workers=os.cpu_count())
+    got = out[0][torch.from_numpy(idx).cuda()].cpu().numpy()
+    assert np.abs(got - want).max() <= TOL * np.abs(want).max()
+    _, npts_o = O.nl_histogram(oracle_geom(cfg), oracle_policy(cfg), m["s"], m["theta"], m["mu"])
+    assert npts == npts_o

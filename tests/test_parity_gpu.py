@@ -159,12 +159,16 @@ def test_binning_is_a_sort(oracle_results):
     assert (np.diff(cs.astype(np.int64)) == hist).all(), "cell_start must be the exclusive scan"
     # every record sits inside its own cell's range
     assert (cs[key_out] <= np.arange(n)).all() and (np.arange(n) < cs[key_out + 1]).all()
-    # multiset of markers preserved (all six fields, bit for bit) and padding is zero
+    # multiset of markers preserved (all six fields, bit for bit)
     src = np.stack([m[f] for f in W.FIELDS], axis=1)
     order_in = np.lexsort(src.T[::-1])
     order_out = np.lexsort(rec[:, :6].T[::-1])
     assert (src[order_in].view(np.uint64) == rec[order_out, :6].view(np.uint64)).all()
-    assert (rec[:, 6:] == 0).all()
+    # slot 6 carries the marker's index in bound order (what orb_gather writes results back by)
+    orig = rec[:, 6].copy().view(np.int64)
+    assert (np.sort(orig) == np.arange(n)).all()
+    assert (src[orig].view(np.uint64) == rec[:, :6].view(np.uint64)).all()
+    assert (rec[:, 7] == 0).all()
     rho_a, _, _ = run_gpu(cfg, m, bin_first=True)
     assert_parity(rho_a, rho_o)
 
