@@ -140,11 +140,13 @@ k_gather_direct(const Params P, const Markers M, const Fields<F> fl,
 }
 
 template <int F>
-__global__ void __launch_bounds__(kThreads)
+__global__ void __launch_bounds__(kThreads, 3)
 k_gather_tile(const Params P, const Markers M, const uint32_t* __restrict__ cell_start,
               const Fields<F> fl, unsigned long long* __restrict__ d_points) {
-  constexpr int kChan = 4 * F;
-  __shared__ __align__(16) double tile[kNH * kNW * kChan];   // [node row][node col][field*4 + plane]
+    // [field][node row][node col][plane], the two 16-byte halves of a node swapped on every other
+  // group of 4 nodes: lanes of a quarter-warp read the same half of (mostly) different nodes, and
+  // the swap spreads them over all eight 16-byte bank groups instead of four
+  __shared__ __align__(16) double tile[F * kNH * kNW * 4];
   __shared__ uint32_t row_begin[kTileI], row_off[kTileI + 1];
   const int tid = threadIdx.x;
   const int tj = blockIdx.x, ti = blockIdx.y, k = blockIdx.z;
@@ -191,9 +193,10 @@ k_gather_tile(const Params P, const Markers M, const uint32_t* __restrict__ cell
 #pragma unroll
       for (int d = 0; d < 4; ++d) v[d] = __ldg(src + wrap_index(k - 1 + d, P.nph));
     }
-    double2* dst = reinterpret_cast<double2*>(tile + node * kChan + f * 4);
-    dst[0] = make_double2(v[0], v[1]);
-    dst[1] = make_double2(v[2], v[3]);
+    double2* dst = reinterpret_cast<double2*>(tile + (f * kNH * kNW + node) * 4);
+    const int sw = (node >> 2) & 1;
+    dst[sw] = make_double2(v[0], v[1]);
+    dst[sw ^ 1] = make_double2(v[2], v[3]);
   }
   __syncthreads();
 
@@ -242,16 +245,18 @@ k_gather_tile(const Params P, const Markers M, const uint32_t* __restrict__ cell
           cardinal_weights(t_s, ws);
         }
         cardinal_weights(t_t, wt);
-        const double* base = tile + (lr * kNW + lc) * kChan;
+        const int node0 = lr * kNW + lc;
 #pragma unroll
         for (int a = 0; a < 4; ++a) {
 #pragma unroll
           for (int b = 0; b < 4; ++b) {
             const double w = ws[a] * wt[b];
-            const double2* nd = reinterpret_cast<const double2*>(base + (a * kNW + b) * kChan);
+            const int node = node0 + a * kNW + b;
+            const int sw = (node >> 2) & 1;
+            const double2* nd = reinterpret_cast<const double2*>(tile) + node * 2;
 #pragma unroll
             for (int f = 0; f < F; ++f) {
-              const double2 lo = nd[2 * f], hi = nd[2 * f + 1];
+              const double2 lo = nd[f * kNH * kNW * 2 + sw], hi = nd[f * kNH * kNW * 2 + (sw ^ 1)];
               acc[f][0] = fma(w, lo.x, acc[f][0]);
               acc[f][1] = fma(w, lo.y, acc[f][1]);
               acc[f][2] = fma(w, hi.x, acc[f][2]);
