@@ -48,9 +48,28 @@ L2_BYTES = 126 << 20
 FP64_MEASURED_TFLOPS = 35.8    # fallback if the live probe (orb_probe_dfma) fails
 FP64_NOMINAL_TFLOPS = 37.2
 
-# dram__bytes_read.sum + dram__bytes_write.sum of ONE launch of the deposit kernel, from the
-# `ncu --set full` capture summarised in profiles/ (None until a capture of that workload exists)
-NCU_TRAFFIC_BYTES = {"cfg3": 5075555000 + 758216192}   # profiles/r01_final_deposit_ncu.md
+TRAFFIC_JSON = os.path.join(ROOT, "profiles", "r02_traffic.json")
+
+
+def ncu_traffic(workload: str, kernel: str):
+    """dram__bytes_read.sum + dram__bytes_write.sum of ONE launch of the dominant kernel, from the
+    committed `ncu --set full` capture (profiles/r02_traffic.json, written by
+    `python -m paper_1908_02219_b200.profile_traffic`).  Keyed by workload AND by the hash of the
+    kernel sources: a capture of other sources is stale and reads as null, with the reason."""
+    from paper_1908_02219_b200 import profile_traffic as PT
+    try:
+        with open(TRAFFIC_JSON) as f:
+            db = json.load(f)
+    except Exception:  # noqa: BLE001
+        return None, "no capture committed (profiles/r02_traffic.json missing)"
+    e = db.get("entries", {}).get(workload)
+    if not e:
+        return None, "no ncu capture of workload %s" % workload
+    if e.get("kernel_source_sha16") != PT.kernel_source_hash():
+        return None, "stale: kernel sources changed since the capture (%s)" % e.get("captured", "?")
+    if kernel not in e.get("kernel", ""):
+        return None, "capture is of %s, not %s" % (e.get("kernel"), kernel)
+    return int(e["dram_bytes"]), "profiles/r02_traffic.json (%s)" % e.get("source", "")
 
 
 def measured_hbm_peak():
@@ -122,16 +141,24 @@ def pick_config(name: str, rank: int):
     return dataclasses.replace(cfg, seed=R.replica_seed(cfg.seed, rank))
 
 
-def config_json(cfg, world, extra=None):
-    c = {"workload": "%s: grid %dx%dx%d cells, %d markers fp64 SoA, %s N_L%s, rho_star=1/%d, %s, %s order"
-         % (cfg.name, cfg.ns, cfg.ntheta, cfg.nphi, cfg.n_markers,
-            "adaptive" if cfg.adaptive else "fixed",
-            ("=4..%d" % cfg.n_max) if cfg.adaptive else ("=%d" % cfg.n_fixed),
-            round(1 / cfg.rho_star), "rho+jpar" if cfg.current else "rho only", cfg.order),
-         "step": "bind + bin (counting sort by cell) + zero grids + tile deposit",
+def describe(cfg):
+    return ("%s: grid %dx%dx%d cells, %d markers fp64 SoA, %s N_L%s, rho_star=1/%d, q=%g, %s, %s order"
+            % (cfg.name, cfg.ns, cfg.ntheta, cfg.nphi, cfg.n_markers,
+               "adaptive" if cfg.adaptive else "fixed",
+               ("=%d..%d" % (cfg.n_fixed, cfg.n_max)) if cfg.adaptive else ("=%d" % cfg.n_fixed),
+               round(1 / cfg.rho_star), cfg.q, "rho+jpar" if cfg.current else "rho only", cfg.order))
+
+
+def config_json(cfgs, world, workload=None, extra=None):
+    if not isinstance(cfgs, (list, tuple)):
+        cfgs = [cfgs]
+    c = {"workload": " + ".join(describe(x) for x in cfgs) if len(cfgs) > 1 else describe(cfgs[0]),
+         "step": "per species: bind + bin (counting sort by cell) + tile deposit; grids zeroed once",
          "l2_policy": "inputs (%.2f GB markers) larger than the 126 MB L2; no flush needed"
-                      % (cfg.n_markers * 48 / 1e9),
+                      % (sum(x.n_markers for x in cfgs) * 48 / 1e9),
          "parallelism": "replicas x%d (no sharding, no collective)" % world if world > 1 else "1 GPU"}
+    if workload:
+        c["name"] = workload
     if extra:
         c.update(extra)
     return c
@@ -160,7 +187,7 @@ def run_reference(args):
     rank, _, world = R.env_rank()
     if rank != 0:
         return 0
-    cfg = pick_config(args.workload, 0)
+    cfg = pick_config(W.WORKLOADS[args.workload][0], 0)
     n_sample = min(args.ref_sample, cfg.n_markers)
     m = W.generate(W.scaled(cfg, n_sample))
     for _ in range(args.warmup):
@@ -177,7 +204,7 @@ def run_reference(args):
         "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
         "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * secs / args.steps,
         "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
-        "data": "synthetic", "config": config_json(cfg, 1, {"step": "oracle_deposit on a bounded sample"}),
+        "data": "synthetic", "config": config_json(cfg, 1, args.workload, {"step": "oracle_deposit on a bounded sample"}),
         "cpu_baseline": {"value": value, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample},
         "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0, "host_cores": os.cpu_count(),
@@ -187,6 +214,31 @@ def run_reference(args):
 
 
 # ------------------------------------------------------------------------------------------
+class Species:
+    """One marker species of the workload: pinned host arrays, device copies, its grid handle."""
+
+    def __init__(self, cfg, dev, local_rank, B, torch):
+        self.cfg = cfg
+        n = cfg.n_markers
+        self.host = {f: torch.empty(n, dtype=torch.float64, pin_memory=True) for f in W.FIELDS}
+        self.m = {f: self.host[f].numpy() for f in W.FIELDS}
+        W.generate(cfg, out=self.m)
+        self.d = {f: self.host[f].to(dev, non_blocking=True) for f in W.FIELDS}
+        self.g = B.grid_for(cfg, device=local_rank)
+        self.pol = B.policy_for(cfg)
+        self.bind_flags = B.ORB_MARKERS_SORTED if cfg.order == "sorted" else 0
+
+    def bind(self):
+        d, cfg = self.d, self.cfg
+        self.g.markers_bind(d["s"], d["theta"], d["phi"], d["vpar"] if cfg.current else None, d["mu"],
+                            d["w"], flags=self.bind_flags)
+
+
+def deposit_kernel_name(cfg):
+    """The tile kernel orb_deposit picks for this N_L policy (csrc/orb_api.cu)."""
+    return "k_deposit_tile" if (cfg.adaptive or cfg.n_fixed > 4) else "k_deposit_ws"
+
+
 def run_ours(args):
     import torch
 
@@ -211,50 +263,47 @@ def run_ours(args):
     except Exception:  # noqa: BLE001
         fp64_peak, fp64_src = FP64_MEASURED_TFLOPS, "profiles/r01_microbench.md"
 
-    cfg = pick_config(args.workload, rank)
-    n = cfg.n_markers
     # inputs: generated on the host into pinned memory (they are the e2e leg's source)
-    host = {f: torch.empty(n, dtype=torch.float64, pin_memory=True) for f in W.FIELDS}
-    m = {f: host[f].numpy() for f in W.FIELDS}
-    W.generate(cfg, out=m)
-    d = {f: host[f].to(dev, non_blocking=True) for f in W.FIELDS}
+    cfgs = [pick_config(name, rank) for name in W.WORKLOADS[args.workload]]
+    species = [Species(c, dev, local_rank, B, torch) for c in cfgs]
     torch.cuda.synchronize()
-
-    g = B.grid_for(cfg, device=local_rank)
-    shape = g.shape()
+    cfg = cfgs[0]                     # grid shape and outputs are common to the species
+    current = any(c.current for c in cfgs)
+    shape = species[0].g.shape()
     rho = torch.zeros(shape, dtype=torch.float64, device=dev)
-    jpar = torch.zeros(shape, dtype=torch.float64, device=dev) if cfg.current else None
-    pol = B.policy_for(cfg)
-    bind_flags = B.ORB_MARKERS_SORTED if cfg.order == "sorted" else 0
+    jpar = torch.zeros(shape, dtype=torch.float64, device=dev) if current else None
     stream = torch.cuda.current_stream()
     st = stream.cuda_stream
+    NS = len(species)
 
     def step(evs=None):
-        g.markers_bind(d["s"], d["theta"], d["phi"], d["vpar"] if cfg.current else None, d["mu"],
-                       d["w"], flags=bind_flags)
-        if evs:
-            evs[0].record(stream)
-        g.markers_bin(st)
-        if evs:
-            evs[1].record(stream)
-        g.grid_zero(rho, jpar, st)
-        if evs:
-            evs[2].record(stream)
-        g.deposit(rho, jpar, pol, st)
-        if evs:
-            evs[3].record(stream)
+        for i, sp in enumerate(species):
+            sp.bind()
+            if evs:
+                evs[4 * i + 0].record(stream)
+            sp.g.markers_bin(st)
+            if evs:
+                evs[4 * i + 1].record(stream)
+            if i == 0:
+                sp.g.grid_zero(rho, jpar, st)
+            if evs:
+                evs[4 * i + 2].record(stream)
+            sp.g.deposit(rho, jpar if sp.cfg.current else None, sp.pol, st)
+            if evs:
+                evs[4 * i + 3].record(stream)
 
     for _ in range(args.warmup):
         step()
     torch.cuda.synchronize()
-    npts_step = g.last_points()
-    fallback_step = g.last_fallback_points()
+    npts_sp = [sp.g.last_points() for sp in species]
+    npts_step = sum(npts_sp)
+    fallback_step = sum(sp.g.last_fallback_points() for sp in species)
 
     K = args.steps
-    evs = [[torch.cuda.Event(enable_timing=True) for _ in range(4)] for _ in range(K)]
+    evs = [[torch.cuda.Event(enable_timing=True) for _ in range(4 * NS)] for _ in range(K)]
     e_start, e_end = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     sampler = ClockSampler(index=local_rank)
-    launches0 = g.launch_count()
+    launches0 = sum(sp.g.launch_count() for sp in species)
     R.barrier()
     torch.cuda.synchronize()
     sampler.start()
@@ -265,38 +314,80 @@ def run_ours(args):
     torch.cuda.synchronize()
     R.barrier()
     sampler.stop()
-    launches = g.launch_count() - launches0
+    launches = sum(sp.g.launch_count() for sp in species) - launches0
     total_ms = e_start.elapsed_time(e_end)
-    bin_ms = sum(e[0].elapsed_time(e[1]) for e in evs) / K
+    bin_ms = sum(e[4 * i].elapsed_time(e[4 * i + 1]) for e in evs for i in range(NS)) / K
     zero_ms = sum(e[1].elapsed_time(e[2]) for e in evs) / K
-    dep_ms_all = [e[2].elapsed_time(e[3]) for e in evs]
+    dep_sp = [[e[4 * i + 2].elapsed_time(e[4 * i + 3]) for e in evs] for i in range(NS)]
+    dep_ms_all = [sum(dep_sp[i][k] for i in range(NS)) for k in range(K)]
     dep_ms = sum(dep_ms_all) / K
-    assert g.last_points() == npts_step
+    assert sum(sp.g.last_points() for sp in species) == npts_step
 
     # result sanity inside the bench: charge conservation (P1) of the last step
     q_sum = float(rho.sum().item())
-    w_sum = float(d["w"].sum().item()) * cfg.q
-    w_abs = float(d["w"].abs().sum().item()) * abs(cfg.q)
+    w_sum = sum(float(sp.d["w"].sum().item()) * sp.cfg.q for sp in species)
+    w_abs = sum(float(sp.d["w"].abs().sum().item()) * abs(sp.cfg.q) for sp in species)
     conservation = abs(q_sum - w_sum) / w_abs
 
     job_ms, job_pts = R.combine(total_ms, float(npts_step) * K, device=dev)
     value = job_pts / (job_ms * 1e-3)
 
+    # ---- NEXT-1 leg: get fields + gyroaverage of n_grids fields on the binned markers
+    gather = None
+    if not args.no_gather:
+        nf = 2 if current else 1
+        gen = torch.Generator(device=dev)
+        gen.manual_seed(1234 + rank)
+        fields = [torch.randn(shape, dtype=torch.float64, device=dev, generator=gen) for _ in range(nf)]
+        g_ms, g_pts, g_fb = 0.0, 0, 0
+        for sp in species:
+            outs = [torch.empty(sp.cfg.n_markers, dtype=torch.float64, device=dev) for _ in range(nf)]
+            ge = [torch.cuda.Event(enable_timing=True) for _ in range(2)]
+            for _ in range(3):
+                sp.g.gather(fields, outs, sp.pol, st)
+            ge[0].record(stream)
+            for _ in range(K):
+                sp.g.gather(fields, outs, sp.pol, st)
+            ge[1].record(stream)
+            torch.cuda.synchronize()
+            g_ms += ge[0].elapsed_time(ge[1]) / K
+            g_pts += sp.g.last_points()
+            g_fb += sp.g.last_fallback_points()
+            del outs
+        # what the method must move: s, theta*, phi, mu in and nf results out per marker; every
+        # node of every field read once
+        g_bytes = sum(c.n_markers for c in cfgs) * 8 * (4 + nf) + nf * cfg.nodes * 8
+        gather = {"ms": g_ms, "fields": nf, "points": g_pts, "fallback_points": g_fb,
+                  "algorithmic_bytes": g_bytes}
+        del fields
+        torch.cuda.empty_cache()
+
     # ---- e2e: HOST marker arrays -> orb_deposit_host -> HOST grids, every step
     E = max(1, min(args.e2e_steps, K))
-    rho_h = torch.empty(shape, dtype=torch.float64, pin_memory=True)
-    jpar_h = torch.empty(shape, dtype=torch.float64, pin_memory=True) if cfg.current else None
-    del d
+    rho_h = [torch.empty(shape, dtype=torch.float64, pin_memory=True) for _ in species]
+    jpar_h = [torch.empty(shape, dtype=torch.float64, pin_memory=True) if sp.cfg.current else None
+              for sp in species]
+    for sp in species:
+        sp.d = None
     torch.cuda.empty_cache()
 
     def e2e_step():
-        return g.deposit_host(m["s"], m["theta"], m["phi"], m["vpar"] if cfg.current else None,
-                              m["mu"], m["w"], rho_h.numpy(), jpar_h.numpy() if cfg.current else None,
-                              pol)
+        pts = up = down = 0
+        for i, sp in enumerate(species):
+            m, c = sp.m, sp.cfg
+            a, b, cdown = sp.g.deposit_host(m["s"], m["theta"], m["phi"], m["vpar"] if c.current else None,
+                                            m["mu"], m["w"], rho_h[i].numpy(),
+                                            jpar_h[i].numpy() if c.current else None, sp.pol)
+            pts, up, down = pts + a, up + b, down + cdown
+            if i > 0:      # species add into the same grids: summed on the host
+                rho_h[0].add_(rho_h[i])
+                if c.current and jpar_h[0] is not None:
+                    jpar_h[0].add_(jpar_h[i])
+        return pts, up, down
 
     e2e_step()
     torch.cuda.synchronize()
-    launches_e0 = g.launch_count()
+    launches_e0 = sum(sp.g.launch_count() for sp in species)
     R.barrier()
     torch.cuda.synchronize()
     t0 = time.perf_counter()
@@ -305,40 +396,47 @@ def run_ours(args):
     torch.cuda.synchronize()
     e2e_ms = (time.perf_counter() - t0) * 1e3
     R.barrier()
-    launches_e = g.launch_count() - launches_e0
+    launches_e = sum(sp.g.launch_count() for sp in species) - launches_e0
     e2e_job_ms, e2e_job_pts = R.combine(e2e_ms, float(npts_e) * E, device=dev)
     e2e_value = e2e_job_pts / (e2e_job_ms * 1e-3)
-    e2e_conservation = abs(float(rho_h.sum().item()) - w_sum) / w_abs
-    g.destroy()
+    e2e_conservation = abs(float(rho_h[0].sum().item()) - w_sum) / w_abs
+    for sp in species:
+        sp.g.destroy()
 
     line = None
     if rank == 0:
         peak, peak_src = measured_hbm_peak()
-        alg_bytes = cfg.algorithmic_bytes
+        n_grids = 2 if current else 1
+        alg_bytes = sum(c.n_markers * 8 * (6 if c.current else 5) for c in cfgs) + n_grids * cfg.nodes * 16
         achieved = alg_bytes / (dep_ms * 1e-3) / 1e9
-        flops = 2.0 * 64.0 * (2 if cfg.current else 1) * npts_step
+        flops = sum(2.0 * 64.0 * (2 if c.current else 1) * n for c, n in zip(cfgs, npts_sp))
+        # the dominant kernel: the deposit kernel of the species that takes longest
+        dom = max(range(NS), key=lambda i: sum(dep_sp[i]))
+        kernel = deposit_kernel_name(cfgs[dom])
+        traffic, traffic_src = ncu_traffic(args.workload, kernel)
         line = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K,
             "warmup": args.warmup, "ms_per_step": job_ms / K, "higher_is_better": True,
             "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-            "config": config_json(cfg, world),
+            "config": config_json(cfgs, world, args.workload),
             "points_per_step": npts_step,
             "fallback_points_per_step": fallback_step,
             "phases_ms": {"bin": bin_ms, "zero": zero_ms, "deposit": dep_ms,
-                          "deposit_min": min(dep_ms_all), "deposit_max": max(dep_ms_all)},
+                          "deposit_min": min(dep_ms_all), "deposit_max": max(dep_ms_all),
+                          "deposit_per_species": [sum(x) / K for x in dep_sp]},
             "deposit_only": {"value": npts_step / (dep_ms * 1e-3), "unit": UNIT,
-                             "note": "tile deposit kernel on already-binned markers"},
+                             "note": "tile deposit kernel(s) on already-binned markers"},
             "step_hbm": {"achieved": alg_bytes * K / (total_ms * 1e-3) / 1e9, "unit": "GB/s",
                          "frac": alg_bytes * K / (total_ms * 1e-3) / 1e9 / peak,
                          "note": "same algorithmic bytes over the whole step (bin + zero + deposit)"},
-            "roofline": {"bound": "hbm", "kernel": "k_deposit_tile", "achieved": achieved,
+            "roofline": {"bound": "hbm", "kernel": kernel, "achieved": achieved,
                          "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                         "traffic": NCU_TRAFFIC_BYTES.get(cfg.name), "peak_source": peak_src,
+                         "traffic": traffic, "traffic_source": traffic_src, "peak_source": peak_src,
                          "algorithmic_bytes": alg_bytes, "kernel_ms": dep_ms,
                          "frac_of_nominal_8TBs": achieved / HBM_NOMINAL_GBS,
                          "note": "contract metric of BASELINE.json; the roof that actually binds "
                                  "this path is the fp64 pipe: see roofline_alu (DESIGN.md 6)"},
-            "roofline_alu": {"bound": "alu", "pipe": "fp64", "kernel": "k_deposit_tile",
+            "roofline_alu": {"bound": "alu", "pipe": "fp64", "kernel": kernel,
                              "achieved": flops / (dep_ms * 1e-3) / 1e12, "peak": fp64_peak,
                              "peak_source": fp64_src,
                              "unit": "TFLOP/s",
@@ -356,9 +454,21 @@ def run_ours(args):
             "checks": {"charge_conservation_rel": conservation,
                        "e2e_charge_conservation_rel": e2e_conservation},
         }
+        if gather:
+            g_ach = gather["algorithmic_bytes"] / (gather["ms"] * 1e-3) / 1e9
+            line["gather"] = {
+                "what": "NEXT-1 get fields + gyroaverage (orb_gather) of %d field(s) on the binned "
+                        "markers" % gather["fields"],
+                "value": gather["points"] / (gather["ms"] * 1e-3), "unit": UNIT,
+                "ms": gather["ms"], "fallback_points": gather["fallback_points"],
+                "roofline": {"bound": "hbm", "kernel": "k_gather_tile", "achieved": g_ach, "peak": peak,
+                             "unit": "GB/s", "frac": g_ach / peak, "traffic": None,
+                             "algorithmic_bytes": gather["algorithmic_bytes"],
+                             "note": "4 marker fields in + 1 result out per marker and field, every "
+                                     "node of every field read once"}}
         if world == 1 and not args.no_cpu_baseline:
-            n_sample = min(args.cpu_sample, n)
-            npts_o, secs = oracle_sample(cfg, m, n_sample)
+            n_sample = min(args.cpu_sample, cfg.n_markers)
+            npts_o, secs = oracle_sample(cfg, species[0].m, n_sample)
             line["cpu_baseline"] = {
                 "value": npts_o / secs, "unit": UNIT, "cores": 1, "kind": "oracle",
                 "sample": "first %d markers of %s (%d Larmor points, %.1f s), single thread; host has %d cores"
@@ -376,13 +486,14 @@ def main(argv=None):
     ap.add_argument("--steps", type=int, default=20)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--workload", default="cfg3", choices=sorted(W.CONFIGS))
+    ap.add_argument("--workload", default="cfg3", choices=sorted(W.WORKLOADS))
     ap.add_argument("--e2e-steps", type=int, default=3)
     ap.add_argument("--cpu-sample", type=int, default=1 << 21,
                     help="markers of the workload the cpu_baseline leg times the oracle on")
     ap.add_argument("--ref-sample", type=int, default=1 << 18,
                     help="markers per step of the --impl reference arm")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-gather", action="store_true", help="skip the orb_gather (NEXT-1) leg")
     args = ap.parse_args(argv)
     if args.warmup < 3 and args.impl == "ours":
         print("bench.py: note: fewer than 3 warm-up steps requested", file=sys.stderr)

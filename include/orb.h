@@ -86,9 +86,13 @@ enum { ORB_NL_FIXED = 0, ORB_NL_ADAPTIVE = 1 };
 #define ORB_DEPOSIT_ALGO_ATOMIC 0x4u /* use the one-thread-per-marker global-atomics kernel
                                         (the GPU algorithm of) instead of the
                                         shared-memory tile kernel                              */
-#define ORB_DEPOSIT_ALGO_TILE_V4 0x8u /* use the round-1 tile kernel (one block per tile, all
-                                        warps run all phases) instead of the persistent
-                                        warp-specialised one; kept for comparison               */
+#define ORB_DEPOSIT_ALGO_TILE_V4 0x8u /* force the one-block-per-tile kernel (all warps run all
+                                        phases; several blocks per SM)                          */
+#define ORB_DEPOSIT_ALGO_TILE_WS 0x10u /* force the persistent warp-specialised tile kernel
+                                        (producer / consumer warps, one block per SM)
+                                        By default the library picks between the two tile
+                                        kernels by N_L policy: persistent for fixed N_L <= 4,
+                                        one-block-per-tile for larger or adaptive N_L.            */
 
 /* Number of Larmor points per marker (R7-R9):
  *   FIXED:    N_L = n_fixed
@@ -108,6 +112,12 @@ typedef struct {
 #define ORB_MARKERS_SORTED 0x1u /* markers are already sorted by guiding-centre cell key
                                    (k_phi*ns + i_s)*ntheta + j_theta (non-decreasing; R17);
                                    binning then only locates the cell boundaries            */
+
+#define ORB_MARKERS_TILE_BINS 0x2u /* bin into slack tile bins (one fixed-capacity segment of records
+                                     per 8 x 16-cell tile and toroidal slab, ~2x the dense layout's
+                                     memory) so that the binning can be refreshed incrementally
+                                     with orb_markers_rebin.  Excludes
+                                     ORB_MARKERS_SORTED.  At most ~1600 markers per tile on average. */
 
 /* Creates a handle for one grid on desc->device and allocates nothing that
  * scales with the marker count yet.  *out is written only on success. */
@@ -176,6 +186,43 @@ int orb_deposit(orb_grid_t *g, double *rho, double *jpar, const orb_nl_policy_t 
 int orb_gather(orb_grid_t *g, int32_t n_fields, const double *const *fields, double *const *out,
                const orb_nl_policy_t *policy, void *stream);
 
+/* ---- Incremental re-binning.  PAPER.md:169-173: the bucket sort is "the most
+ * time-consuming part" and cancels the gain it brings to the deposit; PAPER.md:235 proposes to
+ * track the markers that leave their cell instead of sorting from scratch.  For markers bound with
+ * ORB_MARKERS_TILE_BINS the library keeps its binned copy in slack tile bins: orb_markers_bin
+ * builds them in ONE pass; after the markers have moved, orb_markers_rebin relocates only those that
+ * left their tile.  The binned records are the data the deposit and gather kernels read, so the
+ * new coordinates must reach them first: either orb_markers_refresh (copies the current values of
+ * the six bound arrays into the records) or a pusher that updates the records in place
+ * (orb_markers_layout).  Deposits are then identical to those after a fresh orb_markers_bin up
+ * to summation order; a marker that ends in a neighbouring tile (full tile, full mover buffer) only
+ * costs speed.  All three calls are asynchronous on `stream` and never allocate. */
+
+/* records <- current values of the bound arrays (every marker; 64-byte record writes). */
+int orb_markers_refresh(orb_grid_t *g, void *stream);
+
+/* Re-derives every record's tile from its (s, theta*, phi); moves the records that left their tile
+ * (one 32-byte read per marker + 256 bytes per mover).  ORB_E_STATE unless the markers are bound with
+ * ORB_MARKERS_TILE_BINS and binned. */
+int orb_markers_rebin(orb_grid_t *g, void *stream);
+
+/* Markers moved by the last orb_markers_rebin, and (optional) movers left in place because the
+ * mover buffer (n/2 records) was full -- they move at the next rebin.  Synchronises the device. */
+int orb_last_moved(orb_grid_t *g, int64_t *n_moved, int64_t *n_left_in_place);
+
+/* Where the binned records live, for a pusher that updates them in place (DEVICE pointers, owned by
+ * the library, valid until the next bind/destroy): record r of tile t is records[(t*capacity + r) *
+ * record_doubles + {0: s, 1: theta*, 2: phi, 3: vpar, 4: mu, 5: w, 6: index in bound order (int64
+ * bits), 7: 0}], r < min(count[t], capacity); tile t = (k_phi*tiles_s + i_s/8)*tiles_theta + j_theta/16. */
+typedef struct {
+  double *records;
+  const uint32_t *count;
+  int32_t record_doubles;
+  uint32_t capacity, n_tiles;
+  int32_t tiles_s, tiles_theta;
+} orb_marker_layout_t;
+int orb_markers_layout(const orb_grid_t *g, orb_marker_layout_t *out);
+
 /* Zeroes rho and, if not NULL, jpar (DEVICE arrays of orb_grid_shape doubles) on `stream`
  * (two cudaMemsetAsync; no kernel).  Equivalent to ORB_DEPOSIT_ZERO_FIRST, offered as a call of
  * its own so that a harness can time the deposit kernels apart from the zeroing. */
@@ -231,6 +278,10 @@ int orb_debug_counters(orb_grid_t *g, uint64_t out[16]);
  * ORB_E_STATE if the markers are not binned.  Synchronises the device. */
 int orb_debug_binned(orb_grid_t *g, double *rec_host, uint32_t *cell_start_host,
                      int32_t *rec_doubles);
+
+/* Diagnostic, slack tile bins: count_host (n_tiles uint32) and the records of all tiles, tile by
+ * tile, packed into rec_host (n * 8 doubles).  Meant for small cases (one copy per tile). */
+int orb_debug_tilebins(orb_grid_t *g, double *rec_host, uint32_t *count_host);
 
 /* Host-only diagnostic, no device needed: the polynomial pieces of the clamped (open knot
  * vector) radial cubic B-splines that the tile kernel evaluates (R11).

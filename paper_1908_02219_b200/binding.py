@@ -17,13 +17,16 @@ ORB_DEPOSIT_ZERO_FIRST = 0x1
 ORB_DEPOSIT_NO_BIN = 0x2
 ORB_DEPOSIT_ALGO_ATOMIC = 0x4
 ORB_DEPOSIT_ALGO_TILE_V4 = 0x8
+ORB_DEPOSIT_ALGO_TILE_WS = 0x10
 ORB_MARKERS_SORTED = 0x1
+ORB_MARKERS_TILE_BINS = 0x2
 ORB_MAX_NL = 32
 ORB_MAX_FIELDS = 8
 
 # every symbol include/orb.h declares
 SYMBOLS = ("orb_grid_create", "orb_grid_destroy", "orb_grid_shape", "orb_markers_bind",
-           "orb_reserve", "orb_markers_bin", "orb_deposit", "orb_gather", "orb_grid_zero", "orb_last_points", "orb_last_fallback_points", "orb_deposit_host",
+           "orb_reserve", "orb_markers_bin", "orb_markers_refresh", "orb_markers_rebin", "orb_last_moved",
+           "orb_markers_layout", "orb_debug_tilebins", "orb_deposit", "orb_gather", "orb_grid_zero", "orb_last_points", "orb_last_fallback_points", "orb_deposit_host",
            "orb_launch_count", "orb_debug_counters", "orb_debug_binned", "orb_probe_dfma", "orb_spline_table_radial", "orb_strerror", "orb_last_error", "orb_version")
 
 
@@ -45,6 +48,12 @@ class NlPolicy(C.Structure):
                 ("flags", C.c_uint32), ("rho_ref", C.c_double), ("alpha0", C.c_double)]
 
 
+class MarkerLayout(C.Structure):
+    _fields_ = [("records", C.c_void_p), ("count", C.c_void_p), ("record_doubles", C.c_int32),
+                ("capacity", C.c_uint32), ("n_tiles", C.c_uint32), ("tiles_s", C.c_int32),
+                ("tiles_theta", C.c_int32)]
+
+
 _lib = None
 
 
@@ -64,6 +73,11 @@ def lib():
     L.orb_markers_bind.argtypes = [vp, C.c_int64, dp, dp, dp, dp, dp, dp, C.c_uint32]
     L.orb_reserve.argtypes = [vp, C.c_int64]
     L.orb_markers_bin.argtypes = [vp, vp]
+    L.orb_markers_refresh.argtypes = [vp, vp]
+    L.orb_markers_rebin.argtypes = [vp, vp]
+    L.orb_last_moved.argtypes = [vp, i64p, i64p]
+    L.orb_markers_layout.argtypes = [vp, C.POINTER(MarkerLayout)]
+    L.orb_debug_tilebins.argtypes = [vp, dp, dp]
     L.orb_deposit.argtypes = [vp, dp, dp, C.POINTER(NlPolicy), vp]
     L.orb_gather.argtypes = [vp, C.c_int32, C.POINTER(C.c_void_p), C.POINTER(C.c_void_p),
                              C.POINTER(NlPolicy), vp]
@@ -152,6 +166,32 @@ class Grid:
 
     def markers_bin(self, stream=None):
         _check(lib().orb_markers_bin(self._h, stream), self._h)
+
+    def markers_refresh(self, stream=None):
+        _check(lib().orb_markers_refresh(self._h, stream), self._h)
+
+    def markers_rebin(self, stream=None):
+        _check(lib().orb_markers_rebin(self._h, stream), self._h)
+
+    def last_moved(self):
+        """-> (markers moved by the last rebin, movers left in place)."""
+        a, b = C.c_int64(), C.c_int64()
+        _check(lib().orb_last_moved(self._h, C.byref(a), C.byref(b)), self._h)
+        return a.value, b.value
+
+    def markers_layout(self) -> MarkerLayout:
+        out = MarkerLayout()
+        _check(lib().orb_markers_layout(self._h, C.byref(out)), self._h)
+        return out
+
+    def debug_tilebins(self, n):
+        """-> (records (n, 8) packed tile by tile, count per tile)."""
+        import numpy as np
+        lay = self.markers_layout()
+        cnt = np.empty(lay.n_tiles, dtype=np.uint32)
+        rec = np.zeros((n, 8), dtype=np.float64)
+        _check(lib().orb_debug_tilebins(self._h, rec.ctypes.data, cnt.ctypes.data), self._h)
+        return rec, cnt
 
     def deposit(self, rho, jpar, pol: NlPolicy, stream=None):
         _check(lib().orb_deposit(self._h, _ptr(rho), _ptr(jpar), C.byref(pol), stream), self._h)

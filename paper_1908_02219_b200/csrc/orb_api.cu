@@ -38,6 +38,18 @@ struct orb_grid {
   bool dep_event_valid;
   int sms;                   // multiprocessors of the device
 
+  // slack tile bins (ORB_MARKERS_TILE_BINS; orb_tilebin.cu), owned
+  bool tile_mode;            // the current binding uses them
+  TileBins tb;               // geometry of the bins; tb.count aliases tb_count
+  uint32_t* tb_count;
+  int64_t tb_count_capacity; // tiles
+  double* tb_rec;
+  int64_t tb_rec_capacity;   // records
+  double* tb_movers;
+  int64_t tb_mv_capacity;    // records
+  uint32_t* tb_mv_count;
+  unsigned long long* tb_counters;   // [0] movers of the last rebin, [1] movers left in place
+
   // orb_deposit_host staging (owned)
   double* hbuf[6];
   int64_t hbuf_capacity;
@@ -168,7 +180,70 @@ int ensure_bin_scratch(orb_grid* g, int64_t n) {
   return ORB_OK;
 }
 
+void free_tilebins(orb_grid* g) {
+  cudaFree(g->tb_count);
+  cudaFree(g->tb_rec);
+  cudaFree(g->tb_movers);
+  cudaFree(g->tb_mv_count);
+  cudaFree(g->tb_counters);
+  g->tb_count = nullptr;
+  g->tb_rec = nullptr;
+  g->tb_movers = nullptr;
+  g->tb_mv_count = nullptr;
+  g->tb_counters = nullptr;
+  g->tb_count_capacity = g->tb_rec_capacity = g->tb_mv_capacity = 0;
+}
+
+// geometry and scratch of the slack tile bins for n markers (called from orb_markers_bind)
+int ensure_tilebins(orb_grid* g, int64_t n) {
+  TileBins T;
+  T.tiles_i = (g->desc.ns + 7) / 8;
+  T.tiles_j = (g->desc.ntheta + 15) / 16;
+  const int64_t n_tiles = (int64_t)T.tiles_i * T.tiles_j * g->desc.nphi;
+  if (n_tiles >= ((int64_t)1 << 31)) return fail(g, ORB_E_INVAL, "too many tiles");
+  T.n_tiles = (uint32_t)n_tiles;
+  const int64_t mean = (n + n_tiles - 1) / n_tiles;
+  int64_t cap = (2 * mean + 128 + 7) & ~(int64_t)7;
+  if (cap > 2048) cap = 2048;   // one warp compacts a tile with a 64-bit mask per lane
+  if (mean + mean / 4 > cap)
+    return fail(g, ORB_E_INVAL, "ORB_MARKERS_TILE_BINS: more than 1638 markers per tile on average");
+  if (n_tiles * cap >= ((int64_t)1 << 32)) return fail(g, ORB_E_INVAL, "tile bins exceed 2^32 records");
+  T.cap = (uint32_t)cap;
+  T.count = nullptr;
+  const int64_t mv = n / 2 + 1024;
+  if (n_tiles > g->tb_count_capacity || n_tiles * cap > g->tb_rec_capacity || mv > g->tb_mv_capacity) {
+    free_tilebins(g);
+    if (cudaMalloc(&g->tb_count, (size_t)n_tiles * sizeof(uint32_t)) != cudaSuccess ||
+        cudaMalloc(&g->tb_rec, (size_t)(n_tiles * cap) * kRecDoubles * sizeof(double)) != cudaSuccess ||
+        cudaMalloc(&g->tb_movers, (size_t)mv * kRecDoubles * sizeof(double)) != cudaSuccess ||
+        cudaMalloc(&g->tb_mv_count, sizeof(uint32_t)) != cudaSuccess ||
+        cudaMalloc(&g->tb_counters, 2 * sizeof(unsigned long long)) != cudaSuccess ||
+        cudaMemset(g->tb_counters, 0, 2 * sizeof(unsigned long long)) != cudaSuccess) {
+      cudaGetLastError();
+      free_tilebins(g);
+      return fail(g, ORB_E_NOMEM, "slack tile bins");
+    }
+    g->tb_count_capacity = n_tiles;
+    g->tb_rec_capacity = n_tiles * cap;
+    g->tb_mv_capacity = mv;
+  }
+  T.count = g->tb_count;
+  g->tb = T;
+  return ORB_OK;
+}
+
 int do_bin(orb_grid* g, cudaStream_t st) {
+  if (g->tile_mode) {
+    Params P = make_params(g, nullptr);
+    Markers M = g->bound;
+    M.rec = nullptr;
+    int l = launch_tilebin_build(P, M, g->tb, g->tb_count, g->tb_rec, st);
+    if (l < 0) return fail(g, ORB_E_CUDA, "tile-bin build launch", cudaGetLastError());
+    g->launches += l;
+    ORB_CUDA(g, cudaGetLastError());
+    g->binned = true;
+    return ORB_OK;
+  }
   const bool presorted = (g->bind_flags & ORB_MARKERS_SORTED) != 0;
   if (!presorted && g->bound.n > g->bin_capacity)
     return fail(g, ORB_E_STATE, "binning scratch missing (bind allocates it)");
@@ -265,6 +340,7 @@ int orb_grid_destroy(orb_grid_t* g) {
   DeviceGuard dg(g->desc.device);
   cudaDeviceSynchronize();
   free_bin(g);
+  free_tilebins(g);
   cudaFree(g->bin.cell_start);
   cudaFree(g->bin.block_sums);
   cudaFree(g->scoef);
@@ -305,17 +381,25 @@ int orb_markers_bind(orb_grid_t* g, int64_t n, const double* s, const double* th
   if (!g) return ORB_E_INVAL;
   if (n < 0) return fail(g, ORB_E_INVAL, "n < 0");
   if (n >= ((int64_t)1 << 32) - 1) return fail(g, ORB_E_INVAL, "n too large");
-  if (flags & ~ORB_MARKERS_SORTED) return fail(g, ORB_E_INVAL, "unknown bind flag");
+  if (flags & ~(ORB_MARKERS_SORTED | ORB_MARKERS_TILE_BINS)) return fail(g, ORB_E_INVAL, "unknown bind flag");
+  if ((flags & ORB_MARKERS_SORTED) && (flags & ORB_MARKERS_TILE_BINS))
+    return fail(g, ORB_E_INVAL, "ORB_MARKERS_SORTED and ORB_MARKERS_TILE_BINS exclude each other");
   if (n > 0 && (!s || !theta || !phi || !mu || !w)) return fail(g, ORB_E_INVAL, "NULL marker array");
   if (!aligned16(s) || !aligned16(theta) || !aligned16(phi) || !aligned16(vpar) ||
       !aligned16(mu) || !aligned16(w))
     return fail(g, ORB_E_INVAL, "marker arrays must be 16-byte aligned");
-  if (!(flags & ORB_MARKERS_SORTED) && n > g->bin_capacity) {
+  if (flags & ORB_MARKERS_TILE_BINS) {
+    DeviceGuard dg(g->desc.device);
+    if (!dg.ok) return fail(g, ORB_E_CUDA, "cudaSetDevice");
+    int rc = ensure_tilebins(g, n);
+    if (rc != ORB_OK) return rc;
+  } else if (!(flags & ORB_MARKERS_SORTED) && n > g->bin_capacity) {
     DeviceGuard dg(g->desc.device);
     if (!dg.ok) return fail(g, ORB_E_CUDA, "cudaSetDevice");
     int rc = ensure_bin_scratch(g, n);
     if (rc != ORB_OK) return rc;
   }
+  g->tile_mode = (flags & ORB_MARKERS_TILE_BINS) != 0;
   g->bound.s = s;
   g->bound.th = theta;
   g->bound.ph = phi;
@@ -365,6 +449,7 @@ int orb_deposit(orb_grid_t* g, double* rho, double* jpar, const orb_nl_policy_t*
   if (rc != ORB_OK) return rc;
   const bool atomic_algo = (pol->flags & ORB_DEPOSIT_ALGO_ATOMIC) != 0;
   const bool tile_v4 = (pol->flags & ORB_DEPOSIT_ALGO_TILE_V4) != 0;
+  const bool tile_v5 = (pol->flags & ORB_DEPOSIT_ALGO_TILE_WS) != 0;
   const bool no_bin = (pol->flags & ORB_DEPOSIT_NO_BIN) != 0;
   if (!no_bin && !atomic_algo && !g->binned) {
     rc = do_bin(g, st);
@@ -381,14 +466,19 @@ int orb_deposit(orb_grid_t* g, double* rho, double* jpar, const orb_nl_policy_t*
   Markers M = g->bound;
   const bool use_binned = g->binned && !no_bin;
   const bool presorted = (g->bind_flags & ORB_MARKERS_SORTED) != 0;
-  if (use_binned && !presorted) M.rec = g->bin.rec;
+  if (use_binned && !presorted) M.rec = g->tile_mode ? g->tb_rec : g->bin.rec;
+  TileBins TB = g->tb;
+  if (!g->tile_mode) TB.count = nullptr;
   int l;
   if (atomic_algo || !use_binned) {
     l = launch_deposit_atomic(P, M, rho, jpar, g->d_points, st);
-  } else if (tile_v4) {
-    l = launch_deposit_tile(P, M, g->bin.cell_start, rho, jpar, g->d_points, st);
+  } else if (tile_v4 || (!tile_v5 && (P.adaptive || P.n_fixed > 4))) {
+    // N_L > 4 or adaptive: the one-block-per-tile kernel, whose point slots are filled by a
+    // prefix sum over the markers, keeps its lanes busier than the persistent kernel's
+    // unit hand-over (measured: cfg2 5.5 vs 7.5 ms, cfg4 70 vs 111 ms)
+    l = launch_deposit_tile(P, M, g->bin.cell_start, TB, rho, jpar, g->d_points, st);
   } else {
-    l = launch_deposit_ws(P, M, g->bin.cell_start, rho, jpar, g->d_points, g->sms, st);
+    l = launch_deposit_ws(P, M, g->bin.cell_start, TB, rho, jpar, g->d_points, g->sms, st);
   }
   if (l < 0) return fail(g, ORB_E_CUDA, "deposit launch", cudaGetLastError());
   g->launches += l;
@@ -432,8 +522,10 @@ int orb_gather(orb_grid_t* g, int32_t n_fields, const double* const* fields, dou
   Params P = make_params(g, pol);
   Markers M = g->bound;
   const bool presorted = (g->bind_flags & ORB_MARKERS_SORTED) != 0;
-  if (!direct && !presorted) M.rec = g->bin.rec;
-  int l = launch_gather(P, M, g->bin.cell_start, n_fields, fields, out, g->d_points, !direct, st);
+  if (!direct && !presorted) M.rec = g->tile_mode ? g->tb_rec : g->bin.rec;
+  TileBins TB = g->tb;
+  if (!g->tile_mode) TB.count = nullptr;
+  int l = launch_gather(P, M, g->bin.cell_start, TB, n_fields, fields, out, g->d_points, !direct, st);
   if (l < 0) return fail(g, ORB_E_CUDA, "gather launch", cudaGetLastError());
   g->launches += l;
   ORB_CUDA(g, cudaGetLastError());
@@ -491,7 +583,8 @@ int orb_debug_counters(orb_grid_t* g, uint64_t out[16]) {
 int orb_debug_binned(orb_grid_t* g, double* rec_host, uint32_t* cell_start_host,
                      int32_t* rec_doubles) {
   if (!g || !cell_start_host || !rec_doubles) return ORB_E_INVAL;
-  if (!g->have_bind || !g->binned) return fail(g, ORB_E_STATE, "orb_debug_binned before binning");
+  if (!g->have_bind || !g->binned || g->tile_mode)
+    return fail(g, ORB_E_STATE, "orb_debug_binned needs markers binned in the dense layout");
   DeviceGuard dg(g->desc.device);
   if (!dg.ok) return fail(g, ORB_E_CUDA, "cudaSetDevice");
   ORB_CUDA(g, cudaDeviceSynchronize());
@@ -502,6 +595,84 @@ int orb_debug_binned(orb_grid_t* g, double* rec_host, uint32_t* cell_start_host,
   if (!presorted && rec_host && g->bound.n > 0)
     ORB_CUDA(g, cudaMemcpy(rec_host, g->bin.rec, (size_t)g->bound.n * kRecDoubles * sizeof(double),
                            cudaMemcpyDeviceToHost));
+  return ORB_OK;
+}
+
+int orb_markers_refresh(orb_grid_t* g, void* stream) {
+  if (!g) return ORB_E_INVAL;
+  if (!g->have_bind || !g->tile_mode || !g->binned)
+    return fail(g, ORB_E_STATE, "orb_markers_refresh needs binned ORB_MARKERS_TILE_BINS markers");
+  DeviceGuard dg(g->desc.device);
+  if (!dg.ok) return fail(g, ORB_E_CUDA, "cudaSetDevice");
+  Markers M = g->bound;
+  M.rec = nullptr;
+  int l = launch_tilebin_refresh(M, g->tb, g->tb_count, g->tb_rec, static_cast<cudaStream_t>(stream));
+  if (l < 0) return fail(g, ORB_E_CUDA, "refresh launch", cudaGetLastError());
+  g->launches += l;
+  ORB_CUDA(g, cudaGetLastError());
+  return ORB_OK;
+}
+
+int orb_markers_rebin(orb_grid_t* g, void* stream) {
+  if (!g) return ORB_E_INVAL;
+  if (!g->have_bind || !g->tile_mode || !g->binned)
+    return fail(g, ORB_E_STATE, "orb_markers_rebin needs binned ORB_MARKERS_TILE_BINS markers");
+  DeviceGuard dg(g->desc.device);
+  if (!dg.ok) return fail(g, ORB_E_CUDA, "cudaSetDevice");
+  cudaStream_t st = static_cast<cudaStream_t>(stream);
+  ORB_CUDA(g, cudaMemsetAsync(g->tb_counters, 0, 2 * sizeof(unsigned long long), st));
+  Params P = make_params(g, nullptr);
+  int l = launch_tilebin_rebin(P, g->tb, g->tb_count, g->tb_rec, g->tb_movers, (uint32_t)g->tb_mv_capacity,
+                               g->tb_mv_count, g->tb_counters, st);
+  if (l < 0) return fail(g, ORB_E_CUDA, "rebin launch", cudaGetLastError());
+  g->launches += l;
+  ORB_CUDA(g, cudaGetLastError());
+  return ORB_OK;
+}
+
+int orb_last_moved(orb_grid_t* g, int64_t* n_moved, int64_t* n_left_in_place) {
+  if (!g || !n_moved) return ORB_E_INVAL;
+  if (!g->tile_mode || !g->tb_counters) return fail(g, ORB_E_STATE, "no slack tile bins");
+  DeviceGuard dg(g->desc.device);
+  unsigned long long v[2] = {0, 0};
+  ORB_CUDA(g, cudaDeviceSynchronize());
+  ORB_CUDA(g, cudaMemcpy(v, g->tb_counters, sizeof(v), cudaMemcpyDeviceToHost));
+  *n_moved = (int64_t)v[0];
+  if (n_left_in_place) *n_left_in_place = (int64_t)v[1];
+  return ORB_OK;
+}
+
+int orb_markers_layout(const orb_grid_t* g, orb_marker_layout_t* out) {
+  if (!g || !out) return ORB_E_INVAL;
+  if (!g->have_bind || !g->tile_mode) return ORB_E_STATE;
+  out->records = g->tb_rec;
+  out->count = g->tb_count;
+  out->record_doubles = kRecDoubles;
+  out->capacity = g->tb.cap;
+  out->n_tiles = g->tb.n_tiles;
+  out->tiles_s = g->tb.tiles_i;
+  out->tiles_theta = g->tb.tiles_j;
+  return ORB_OK;
+}
+
+int orb_debug_tilebins(orb_grid_t* g, double* rec_host, uint32_t* count_host) {
+  if (!g || !rec_host || !count_host) return ORB_E_INVAL;
+  if (!g->have_bind || !g->tile_mode || !g->binned) return fail(g, ORB_E_STATE, "no binned slack tile bins");
+  DeviceGuard dg(g->desc.device);
+  if (!dg.ok) return fail(g, ORB_E_CUDA, "cudaSetDevice");
+  ORB_CUDA(g, cudaDeviceSynchronize());
+  ORB_CUDA(g, cudaMemcpy(count_host, g->tb_count, (size_t)g->tb.n_tiles * sizeof(uint32_t),
+                         cudaMemcpyDeviceToHost));
+  int64_t off = 0;
+  for (uint32_t t = 0; t < g->tb.n_tiles; ++t) {
+    const uint32_t c = count_host[t] < g->tb.cap ? count_host[t] : g->tb.cap;
+    count_host[t] = c;
+    if (c == 0) continue;
+    if (off + c > g->bound.n) return fail(g, ORB_E_STATE, "tile counts exceed the bound marker count");
+    ORB_CUDA(g, cudaMemcpy(rec_host + off * kRecDoubles, g->tb_rec + (size_t)t * g->tb.cap * kRecDoubles,
+                           (size_t)c * kRecDoubles * sizeof(double), cudaMemcpyDeviceToHost));
+    off += c;
+  }
   return ORB_OK;
 }
 

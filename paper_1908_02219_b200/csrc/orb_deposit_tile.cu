@@ -180,7 +180,7 @@ __device__ __noinline__ void deposit_point_global(const Params& P, double s_l, d
 template <int G, int PCAP>   // G = 1: rho only; G = 2: rho and jpar; PCAP: points per chunk
 __global__ void __launch_bounds__(kThreads, kCtasPerSm)
 k_deposit_tile(const Params P, const Markers M, const uint32_t* __restrict__ cell_start,
-               double* __restrict__ rho, double* __restrict__ jpar,
+               const TileBins TB, double* __restrict__ rho, double* __restrict__ jpar,
                unsigned long long* __restrict__ d_points, int tiles_i, int tiles_j) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   Smem<G, PCAP>& S = *reinterpret_cast<Smem<G, PCAP>*>(smem_raw);
@@ -200,15 +200,11 @@ k_deposit_tile(const Params P, const Markers M, const uint32_t* __restrict__ cel
   if (tid == 0) {
     uint32_t off = 0;
     for (int r = 0; r < kTileI; ++r) {
-      uint32_t b = 0, e = 0;
-      if (i_lo + r < i_hi) {
-        const int64_t c0 = ((int64_t)k * P.ns + (i_lo + r)) * P.nth;
-        b = cell_start[c0 + j_lo];
-        e = cell_start[c0 + j_hi];
-      }
+      uint32_t b, n;
+      tile_run(P, cell_start, TB, tj, ti, k, r, b, n);
       S.row_begin[r] = b;
       S.row_off[r] = off;
-      off += e - b;
+      off += n;
     }
     S.row_off[kTileI] = off;
     S.n_deferred[0] = S.n_deferred[1] = 0;
@@ -609,7 +605,8 @@ k_deposit_tile(const Params P, const Markers M, const uint32_t* __restrict__ cel
 }
 
 template <int G, int PCAP>
-int launch(const Params& P, const Markers& M, const uint32_t* cell_start, double* rho, double* jpar,
+int launch(const Params& P, const Markers& M, const uint32_t* cell_start, const TileBins& TB,
+           double* rho, double* jpar,
            unsigned long long* d_points, cudaStream_t st) {
   const int tiles_i = (P.ns + kTileI - 1) / kTileI;
   const int tiles_j = (P.nth + kTileJ - 1) / kTileJ;
@@ -618,21 +615,22 @@ int launch(const Params& P, const Markers& M, const uint32_t* cell_start, double
   if (cudaFuncSetAttribute(k_deposit_tile<G, PCAP>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                            (int)smem) != cudaSuccess)
     return -1;
-  k_deposit_tile<G, PCAP><<<blocks, kThreads, smem, st>>>(P, M, cell_start, rho, jpar, d_points,
+  k_deposit_tile<G, PCAP><<<blocks, kThreads, smem, st>>>(P, M, cell_start, TB, rho, jpar, d_points,
                                                          tiles_i, tiles_j);
   return 1;
 }
 
 }  // namespace
 
-int launch_deposit_tile(const Params& P, const Markers& M, const uint32_t* cell_start, double* rho,
+int launch_deposit_tile(const Params& P, const Markers& M, const uint32_t* cell_start,
+                        const TileBins& TB, double* rho,
                         double* jpar, unsigned long long* d_points, cudaStream_t st) {
   if (M.n == 0) return 0;
   if (!P.adaptive && P.n_fixed <= 4)
-    return jpar ? launch<2, kPCapSmall>(P, M, cell_start, rho, jpar, d_points, st)
-                : launch<1, kPCapSmall>(P, M, cell_start, rho, jpar, d_points, st);
-  return jpar ? launch<2, kPCapLarge>(P, M, cell_start, rho, jpar, d_points, st)
-              : launch<1, kPCapLarge>(P, M, cell_start, rho, jpar, d_points, st);
+    return jpar ? launch<2, kPCapSmall>(P, M, cell_start, TB, rho, jpar, d_points, st)
+                : launch<1, kPCapSmall>(P, M, cell_start, TB, rho, jpar, d_points, st);
+  return jpar ? launch<2, kPCapLarge>(P, M, cell_start, TB, rho, jpar, d_points, st)
+              : launch<1, kPCapLarge>(P, M, cell_start, TB, rho, jpar, d_points, st);
 }
 
 }  // namespace orb

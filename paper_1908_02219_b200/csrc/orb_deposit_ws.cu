@@ -207,7 +207,7 @@ __device__ __noinline__ void deposit_point_cell(const Params& P, int ci, double 
 // ------------------------------------------------------------------------------------ producer
 template <int G, int PW, int CW, bool SELF>
 __device__ __forceinline__ void producer(Smem<G, PW, CW>& S, const Params& P, const Markers& M,
-                                         const uint32_t* __restrict__ cell_start,
+                                         const uint32_t* __restrict__ cell_start, const TileBins& TB,
                                          double* __restrict__ rho, double* __restrict__ jpar,
                                          unsigned long long* __restrict__ d_points, int tiles_i,
                                          int tiles_j) {
@@ -225,13 +225,7 @@ __device__ __forceinline__ void producer(Smem<G, PW, CW>& S, const Params& P, co
     n = 0;
     if (t < n_tiles && lane < kTileI) {
       const int tj = t % tiles_j, ti = (t / tiles_j) % tiles_i, k = t / (tiles_j * tiles_i);
-      const int i = ti * kTileI + lane;
-      if (i < P.ns) {
-        const int j_lo = tj * kTileJ, j_hi = min(j_lo + kTileJ, P.nth);
-        const int64_t c0 = ((int64_t)k * P.ns + i) * P.nth;
-        b = __ldg(cell_start + c0 + j_lo);
-        n = __ldg(cell_start + c0 + j_hi) - b;
-      }
+      tile_run(P, cell_start, TB, tj, ti, k, lane, b, n);
     }
   };
   // marker v of the tile -> global marker index (lanes hold the descriptor rows)
@@ -752,33 +746,28 @@ __device__ __forceinline__ void consumer(Smem<G, PW, CW>& S, const Params& P,
 
       // The batches of a row segment are contiguous in the sorted order: one linear operand
       // stream, loaded one batch ahead of the MMAs (marker offsets two ahead), across cell
-      // boundaries.  The segment holds at least one batch.
+      // boundaries, in two alternating register sets (A, B) so that no operand is ever copied.
+      // The stream is read up to two batches beyond the segment's end (valid shared memory: the
+      // fields that follow ops / midx in the stage; the values are never used, the marker offsets
+      // are clamped to the table and to 8-byte alignment).
+      constexpr unsigned kMoCap = (unsigned)(Sh::kMCap * kChan * 8);   // the zero marker
       unsigned int pk = St.cs[c_first];
       const char* p = ops_b + (pk & 0xffffu) * 64u;
-      const char* p_end = ops_b + (St.cs[c_first + kSegW] & 0xffffu) * 64u;
       const unsigned short* mi = midx + (pk & 0xffffu);
-      double n_ws = *reinterpret_cast<const double*>(p);
-      double n_w0 = *reinterpret_cast<const double*>(p + wo0);
-      double n_w1 = *reinterpret_cast<const double*>(p + wo1);
-      double n_b = 0.0;
-      if (G == 2 || g < 4) n_b = *reinterpret_cast<const double*>(mt_b + mi[0]);
-      unsigned int n_mo = (p + 256 < p_end) ? mi[4] : 0u;
-
-#define ORB_BATCH                                                                     \
+      double Aw, Ax0, Ax1, Ab = 0.0, Bw, Bx0, Bx1, Bb = 0.0;
+#define ORB_LD(S, q, off)                                                             \
+      S##w = *reinterpret_cast<const double*>((q));                                   \
+      S##x0 = *reinterpret_cast<const double*>((q) + wo0);                            \
+      S##x1 = *reinterpret_cast<const double*>((q) + wo1);                            \
+      if (G == 2 || g < 4) S##b = *reinterpret_cast<const double*>(mt_b + (off));
+#define ORB_MMA(S)                                                                    \
       {                                                                               \
-        const double a0 = n_ws * n_w0, a1 = n_ws * n_w1, bb = n_b;                    \
-        p += 256;                                                                     \
-        mi += 4;                                                                      \
-        if (p < p_end) {                                                              \
-          n_ws = *reinterpret_cast<const double*>(p);                                 \
-          n_w0 = *reinterpret_cast<const double*>(p + wo0);                           \
-          n_w1 = *reinterpret_cast<const double*>(p + wo1);                           \
-          if (G == 2 || g < 4) n_b = *reinterpret_cast<const double*>(mt_b + n_mo);   \
-          if (p + 256 < p_end) n_mo = mi[4];                                          \
-        }                                                                             \
-        dmma884(c0a, c0b, a0, bb);                                                    \
-        dmma884(c1a, c1b, a1, bb);                                                    \
+        const double a0 = S##w * S##x0, a1 = S##w * S##x1;                            \
+        dmma884(c0a, c0b, a0, S##b);                                                  \
+        dmma884(c1a, c1b, a1, S##b);                                                  \
       }
+      ORB_LD(A, p, min((unsigned)mi[0] & 0xfff8u, kMoCap))
+      unsigned int mo = min((unsigned)mi[4] & 0xfff8u, kMoCap);
 
       // Column retire, deferred: stepping past cell U of a group of four finishes one node column
       // of the window.  Its two accumulators are parked in registers (t0: the column this lane's
@@ -796,7 +785,24 @@ __device__ __forceinline__ void consumer(Smem<G, PW, CW>& S, const Params& P,
       {                                                                               \
         int nb = (int)(((pk >> 16) + 3u) >> 2);                                       \
         pk = St.cs[c_first + cc + (U) + 1];                                           \
-        for (; nb > 0; --nb) ORB_BATCH                                                \
+        _Pragma("unroll 1") for (; nb >= 2; nb -= 2) {                                \
+          ORB_LD(B, p + 256, mo)                                                      \
+          mo = min((unsigned)mi[8] & 0xfff8u, kMoCap);                                          \
+          ORB_MMA(A)                                                                  \
+          ORB_LD(A, p + 512, mo)                                                      \
+          mo = min((unsigned)mi[12] & 0xfff8u, kMoCap);                                         \
+          ORB_MMA(B)                                                                  \
+          p += 512;                                                                   \
+          mi += 8;                                                                    \
+        }                                                                             \
+        if (nb) {                                                                     \
+          ORB_LD(B, p + 256, mo)                                                      \
+          mo = min((unsigned)mi[8] & 0xfff8u, kMoCap);                                          \
+          ORB_MMA(A)                                                                  \
+          Aw = Bw; Ax0 = Bx0; Ax1 = Bx1; Ab = Bb;                                     \
+          p += 256;                                                                   \
+          mi += 4;                                                                    \
+        }                                                                             \
         ORB_PARK(U)                                                                   \
       }
 
@@ -867,7 +873,8 @@ __device__ __forceinline__ void consumer(Smem<G, PW, CW>& S, const Params& P,
       __syncwarp();
 #undef ORB_PARK
 #undef ORB_CELL
-#undef ORB_BATCH
+#undef ORB_MMA
+#undef ORB_LD
     }
     __syncwarp();
     mbar_arrive(&S.empty[stage]);
@@ -900,7 +907,7 @@ __device__ __forceinline__ void consumer(Smem<G, PW, CW>& S, const Params& P,
 template <int G, int PW, int CW, bool SELF>
 __global__ void __launch_bounds__((PW + CW) * 32, 1)
 k_deposit_ws(const Params P, const Markers M, const uint32_t* __restrict__ cell_start,
-             double* __restrict__ rho, double* __restrict__ jpar,
+             const TileBins TB, double* __restrict__ rho, double* __restrict__ jpar,
              unsigned long long* __restrict__ d_points, int tiles_i, int tiles_j) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   Smem<G, PW, CW>& S = *reinterpret_cast<Smem<G, PW, CW>*>(smem_raw);
@@ -925,15 +932,15 @@ k_deposit_ws(const Params P, const Markers M, const uint32_t* __restrict__ cell_
   }
   __syncthreads();
   if (tid < Sh::kProd) {
-    producer<G, PW, CW, SELF>(S, P, M, cell_start, rho, jpar, d_points, tiles_i, tiles_j);
+    producer<G, PW, CW, SELF>(S, P, M, cell_start, TB, rho, jpar, d_points, tiles_i, tiles_j);
   } else {
     consumer<G, PW, CW>(S, P, rho, jpar, d_points);
   }
 }
 
 template <int G, int PW, int CW, bool SELF>
-int launch(const Params& P, const Markers& M, const uint32_t* cell_start, double* rho, double* jpar,
-           unsigned long long* d_points, int sms, cudaStream_t st) {
+int launch(const Params& P, const Markers& M, const uint32_t* cell_start, const TileBins& TB,
+           double* rho, double* jpar, unsigned long long* d_points, int sms, cudaStream_t st) {
   const int tiles_i = (P.ns + kTileI - 1) / kTileI;
   const int tiles_j = (P.nth + kTileJ - 1) / kTileJ;
   const int64_t n_tiles = (int64_t)tiles_i * tiles_j * P.nph;
@@ -943,23 +950,27 @@ int launch(const Params& P, const Markers& M, const uint32_t* cell_start, double
   if (cudaFuncSetAttribute(k_deposit_ws<G, PW, CW, SELF>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                            (int)smem) != cudaSuccess)
     return -1;
-  k_deposit_ws<G, PW, CW, SELF><<<blocks, (PW + CW) * 32, smem, st>>>(P, M, cell_start, rho, jpar,
+  k_deposit_ws<G, PW, CW, SELF><<<blocks, (PW + CW) * 32, smem, st>>>(P, M, cell_start, TB, rho, jpar,
                                                                       d_points, tiles_i, tiles_j);
   return 1;
 }
 
 }  // namespace
 
-int launch_deposit_ws(const Params& P, const Markers& M, const uint32_t* cell_start, double* rho,
-                      double* jpar, unsigned long long* d_points, int sms, cudaStream_t st) {
+int launch_deposit_ws(const Params& P, const Markers& M, const uint32_t* cell_start,
+                      const TileBins& TB, double* rho, double* jpar, unsigned long long* d_points,
+                      int sms, cudaStream_t st) {
   if (M.n == 0) return 0;
-  constexpr int PW = 8, CW = 8;
+#ifndef ORB_CW
+#define ORB_CW 8
+#endif
+  constexpr int PW = 8, CW = ORB_CW;
   const bool self = !P.adaptive && P.n_fixed <= kPPL;
   if (self)
-    return jpar ? launch<2, PW, CW, true>(P, M, cell_start, rho, jpar, d_points, sms, st)
-                : launch<1, PW, CW, true>(P, M, cell_start, rho, jpar, d_points, sms, st);
-  return jpar ? launch<2, PW, CW, false>(P, M, cell_start, rho, jpar, d_points, sms, st)
-              : launch<1, PW, CW, false>(P, M, cell_start, rho, jpar, d_points, sms, st);
+    return jpar ? launch<2, PW, CW, true>(P, M, cell_start, TB, rho, jpar, d_points, sms, st)
+                : launch<1, PW, CW, true>(P, M, cell_start, TB, rho, jpar, d_points, sms, st);
+  return jpar ? launch<2, PW, CW, false>(P, M, cell_start, TB, rho, jpar, d_points, sms, st)
+              : launch<1, PW, CW, false>(P, M, cell_start, TB, rho, jpar, d_points, sms, st);
 }
 
 }  // namespace orb

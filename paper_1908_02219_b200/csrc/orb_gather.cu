@@ -142,7 +142,7 @@ k_gather_direct(const Params P, const Markers M, const Fields<F> fl,
 template <int F>
 __global__ void __launch_bounds__(kThreads, 3)
 k_gather_tile(const Params P, const Markers M, const uint32_t* __restrict__ cell_start,
-              const Fields<F> fl, unsigned long long* __restrict__ d_points) {
+              const TileBins TB, const Fields<F> fl, unsigned long long* __restrict__ d_points) {
     // [field][node row][node col][plane], the two 16-byte halves of a node swapped on every other
   // group of 4 nodes: lanes of a quarter-warp read the same half of (mostly) different nodes, and
   // the swap spreads them over all eight 16-byte bank groups instead of four
@@ -155,14 +155,8 @@ k_gather_tile(const Params P, const Markers M, const uint32_t* __restrict__ cell
 
   // the tile's markers: one contiguous run per radial row (key phi-major, orb_bin.cu)
   if (tid < kTileI) {
-    const int i = ti * kTileI + tid;
-    uint32_t b = 0, n = 0;
-    if (i < P.ns) {
-      const int j_lo = tj * kTileJ, j_hi = min(j_lo + kTileJ, P.nth);
-      const int64_t c0 = ((int64_t)k * P.ns + i) * P.nth;
-      b = __ldg(cell_start + c0 + j_lo);
-      n = __ldg(cell_start + c0 + j_hi) - b;
-    }
+    uint32_t b, n;
+    tile_run(P, cell_start, TB, tj, ti, k, tid, b, n);
     row_begin[tid] = b;
     row_off[tid + 1] = n;
   }
@@ -296,7 +290,8 @@ k_gather_tile(const Params P, const Markers M, const uint32_t* __restrict__ cell
 }
 
 template <int F>
-int launch(const Params& P, const Markers& M, const uint32_t* cell_start, const double* const* fields,
+int launch(const Params& P, const Markers& M, const uint32_t* cell_start, const TileBins& TB,
+           const double* const* fields,
            double* const* out, unsigned long long* d_points, bool tiled, cudaStream_t st) {
   Fields<F> fl;
   for (int f = 0; f < F; ++f) {
@@ -305,7 +300,7 @@ int launch(const Params& P, const Markers& M, const uint32_t* cell_start, const 
   }
   if (tiled) {
     const dim3 grid((P.nth + kTileJ - 1) / kTileJ, (P.ns + kTileI - 1) / kTileI, P.nph);
-    k_gather_tile<F><<<grid, kThreads, 0, st>>>(P, M, cell_start, fl, d_points);
+    k_gather_tile<F><<<grid, kThreads, 0, st>>>(P, M, cell_start, TB, fl, d_points);
   } else {
     const int64_t blocks = (M.n + kThreads - 1) / kThreads;
     k_gather_direct<F><<<(unsigned int)blocks, kThreads, 0, st>>>(P, M, fl, d_points);
@@ -315,15 +310,16 @@ int launch(const Params& P, const Markers& M, const uint32_t* cell_start, const 
 
 }  // namespace
 
-int launch_gather(const Params& P, const Markers& M, const uint32_t* cell_start, int n_fields,
+int launch_gather(const Params& P, const Markers& M, const uint32_t* cell_start, const TileBins& TB,
+                  int n_fields,
                   const double* const* fields, double* const* out, unsigned long long* d_points,
                   bool tiled, cudaStream_t st) {
   if (M.n == 0) return 0;
   int launches = 0;
   for (int f0 = 0; f0 < n_fields; f0 += 2) {   // two fields per launch (16 accumulators per lane)
     const int nf = n_fields - f0 >= 2 ? 2 : 1;
-    launches += nf == 2 ? launch<2>(P, M, cell_start, fields + f0, out + f0, d_points, tiled, st)
-                        : launch<1>(P, M, cell_start, fields + f0, out + f0, d_points, tiled, st);
+    launches += nf == 2 ? launch<2>(P, M, cell_start, TB, fields + f0, out + f0, d_points, tiled, st)
+                        : launch<1>(P, M, cell_start, TB, fields + f0, out + f0, d_points, tiled, st);
     d_points = d_points + 2;   // only the first launch counts the points ([2], [3]: scratch)
   }
   return launches;

@@ -54,6 +54,15 @@ struct Markers {
   int64_t n;
 };
 
+// Slack tile bins (orb_tilebin.cu, NEXT-2): tile t = (k * tiles_i + ti) * tiles_j + tj owns the records
+// [t * cap, t * cap + min(count[t], cap)) of Markers::rec.  count == nullptr: the dense cell-sorted
+// layout of orb_bin.cu (per-cell offsets) is in use instead.
+struct TileBins {
+  const uint32_t* count;
+  uint32_t cap, n_tiles;
+  int tiles_i, tiles_j;
+};
+
 // ---- kernels' host-side launchers (each returns the number of kernels it launched, <0 on error)
 int launch_deposit_atomic(const Params& P, const Markers& M, double* rho, double* jpar,
                           unsigned long long* d_points, cudaStream_t st);
@@ -68,17 +77,29 @@ struct BinScratch {
 int launch_bin(const Params& P, const Markers& M, const BinScratch& B, bool presorted,
                cudaStream_t st);
 
-int launch_deposit_tile(const Params& P, const Markers& M, const uint32_t* cell_start, double* rho,
-                        double* jpar, unsigned long long* d_points, cudaStream_t st);
+int launch_deposit_tile(const Params& P, const Markers& M, const uint32_t* cell_start,
+                        const TileBins& TB, double* rho, double* jpar, unsigned long long* d_points,
+                        cudaStream_t st);
 
 // v5: one persistent, warp-specialised block per SM (orb_deposit_ws.cu); sms = multiprocessors
-int launch_deposit_ws(const Params& P, const Markers& M, const uint32_t* cell_start, double* rho,
-                      double* jpar, unsigned long long* d_points, int sms, cudaStream_t st);
+int launch_deposit_ws(const Params& P, const Markers& M, const uint32_t* cell_start,
+                      const TileBins& TB, double* rho, double* jpar, unsigned long long* d_points,
+                      int sms, cudaStream_t st);
 
 // get fields + gyroaverage (orb_gather.cu); fields / out: host arrays of n_fields device pointers
-int launch_gather(const Params& P, const Markers& M, const uint32_t* cell_start, int n_fields,
+int launch_gather(const Params& P, const Markers& M, const uint32_t* cell_start, const TileBins& TB,
+                  int n_fields,
                   const double* const* fields, double* const* out, unsigned long long* d_points,
                   bool tiled, cudaStream_t st);
+
+// slack tile bins: one-pass build, refresh of the records from the bound arrays, incremental rebin
+int launch_tilebin_build(const Params& P, const Markers& M, const TileBins& T, uint32_t* count, double* rec,
+                         cudaStream_t st);
+int launch_tilebin_refresh(const Markers& M, const TileBins& T, const uint32_t* count, double* rec,
+                           cudaStream_t st);
+int launch_tilebin_rebin(const Params& P, const TileBins& T, uint32_t* count, double* rec, double* movers,
+                         uint32_t mv_cap, uint32_t* mv_count, unsigned long long* counters,
+                         cudaStream_t st);
 
 // ring table (cos, sin)(alpha0 + 2 pi l / N), built on the device (orb_ring.cu)
 int launch_ring_table(double2* ring, double alpha0, cudaStream_t st);

@@ -1,0 +1,242 @@
+// Incremental re-binning.  PAPER.md:169-173: the bucket sort pays for
+// itself on the deposit but is "the most time-consuming part" of the run; PAPER.md:235 proposes
+// to "track markers leaving cells" instead of sorting from scratch.  A dense cell-sorted array
+// cannot be updated in place (any insertion shifts everything behind it), so this second binning
+// layout trades memory for updatability:
+//
+//   slack tile bins   the grid's deposit tiles (1 toroidal slab x 8 radial x 16 poloidal cells,
+//                     the unit of work of the tile kernels) each own a fixed-capacity segment
+//                     rec[t * cap .. t * cap + count[t]) of 64-byte marker records, in any order
+//                     (the tile kernels sort a tile's Larmor points on chip anyway, so per-cell
+//                     order inside a tile buys nothing).  cap ~ 2 x the mean occupancy + 128.
+//   build             ONE pass: slot = atomicAdd(count[tile]); no histogram, no scan.
+//   rebin             after the marker coordinates changed in the records (orb_markers_refresh,
+//                     or a pusher writing them in place): one warp per tile re-derives each
+//                     record's tile; markers that left are copied to a mover buffer and the
+//                     segment is compacted (tail records fill the holes); a second kernel
+//                     appends the movers to their new tiles.  Cost: one 32-byte sector per marker
+//                     (s, theta*, phi) + 4 x 64 bytes per mover.
+//
+// Nothing downstream relies on a marker being in the RIGHT tile for correctness, only for speed
+// (points outside a block's tile take the direct global path).  That makes every overflow benign:
+// a full tile sends the marker to the next tile with room; a full mover buffer leaves the marker
+// where it was until the next rebin.
+#include "orb_geom.cuh"
+
+namespace orb {
+
+namespace {
+
+constexpr int kTileI = 8, kTileJ = 16;
+constexpr unsigned kFull = 0xffffffffu;
+
+__device__ __forceinline__ uint32_t tile_of(const Params& P, int tiles_i, int tiles_j, double s, double th,
+                                            double ph) {
+  int i = min(max((int)(s * (double)P.ns), 0), P.ns - 1);
+  int j = (int)(wrap_2pi(th) * P.nth_scale);
+  int k = (int)(wrap_2pi(ph) * P.nph_scale);
+  j = min(max(j, 0), P.nth - 1);
+  k = min(max(k, 0), P.nph - 1);
+  return ((uint32_t)k * (uint32_t)tiles_i + (uint32_t)(i / kTileI)) * (uint32_t)tiles_j +
+         (uint32_t)(j / kTileJ);
+}
+
+// claim a slot in tile t, or in the next tile with room (benign mis-binning, see the header)
+__device__ __forceinline__ int64_t claim_slot(uint32_t* __restrict__ count, uint32_t t, uint32_t n_tiles,
+                                              uint32_t cap) {
+  for (uint32_t probe = 0; probe < n_tiles; ++probe) {
+    const uint32_t slot = atomicAdd(count + t, 1u);   // counts may overshoot cap: readers clamp
+    if (slot < cap) return (int64_t)t * cap + slot;
+    t = t + 1 < n_tiles ? t + 1 : 0;
+  }
+  return -1;   // unreachable: n_tiles * cap > n
+}
+
+__device__ __forceinline__ void store_record(double* __restrict__ out, double s, double th, double ph,
+                                             double vp, double mu, double w, double idx_bits) {
+  asm volatile("st.global.v4.f64 [%0], {%1, %2, %3, %4};" ::"l"(out), "d"(s), "d"(th), "d"(ph), "d"(vp)
+               : "memory");
+  asm volatile("st.global.v4.f64 [%0], {%1, %2, %3, %4};" ::"l"(out + 4), "d"(mu), "d"(w),
+               "d"(idx_bits), "d"(0.0)
+               : "memory");
+}
+
+__global__ void __launch_bounds__(256)
+k_tilebin_build(const Params P, const Markers M, const TileBins T, uint32_t* __restrict__ count,
+                double* __restrict__ rec) {
+  const int64_t p = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (p >= M.n) return;
+  const double s = __ldg(M.s + p), th = __ldg(M.th + p), ph = __ldg(M.ph + p);
+  const uint32_t t = tile_of(P, T.tiles_i, T.tiles_j, s, th, ph);
+  const int64_t dst = claim_slot(count, t, T.n_tiles, T.cap);
+  if (dst < 0) return;
+  store_record(rec + dst * kRecDoubles, s, th, ph, M.vpar ? __ldg(M.vpar + p) : 0.0, __ldg(M.mu + p),
+               __ldg(M.w + p), __longlong_as_double((long long)p));
+}
+
+// records <- current values of the bound arrays (by the original index kept in the record)
+__global__ void __launch_bounds__(256)
+k_tilebin_refresh(const Markers M, const TileBins T, const uint32_t* __restrict__ count,
+                  double* __restrict__ rec) {
+  const uint32_t t = blockIdx.x;
+  const uint32_t n = min(__ldg(count + t), T.cap);
+  for (uint32_t i = threadIdx.x; i < n; i += blockDim.x) {
+    double* r = rec + ((int64_t)t * T.cap + i) * kRecDoubles;
+    const double ib = r[6];
+    const int64_t p = (int64_t)__double_as_longlong(ib);
+    store_record(r, __ldg(M.s + p), __ldg(M.th + p), __ldg(M.ph + p), M.vpar ? __ldg(M.vpar + p) : 0.0,
+                 __ldg(M.mu + p), __ldg(M.w + p), ib);
+  }
+}
+
+// One warp per tile: movers out, segment compacted.  counters[0] += movers extracted,
+// counters[1] += movers left in place because the mover buffer was full.
+constexpr int kWarpsPerBlock = 4;
+constexpr int kMaxIter = 64;    // cap <= 32 * kMaxIter records per tile
+
+__global__ void __launch_bounds__(kWarpsPerBlock * 32)
+k_tilebin_extract(const Params P, const TileBins T, uint32_t* __restrict__ count, double* __restrict__ rec,
+                  double* __restrict__ movers, uint32_t mv_cap, uint32_t* __restrict__ mv_count,
+                  unsigned long long* __restrict__ counters) {
+  __shared__ unsigned short hole[kWarpsPerBlock][32 * kMaxIter / 2 + 32];
+  __shared__ unsigned short tail[kWarpsPerBlock][32 * kMaxIter / 2 + 32];
+  const int wid = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const uint32_t t = blockIdx.x * kWarpsPerBlock + wid;
+  if (t >= T.n_tiles) return;
+  const uint32_t n = min(count[t], T.cap);
+  if (n == 0) {
+    if (lane == 0) count[t] = 0;
+    return;
+  }
+  double* base = rec + (int64_t)t * T.cap * kRecDoubles;
+  const int iters = (int)((n + 31) / 32);
+  // pass 1: who leaves?  bit x of `gone`: record x * 32 + lane is a mover that was copied out
+  unsigned long long gone = 0;
+  uint32_t n_gone = 0, n_kept_back = 0;
+  for (int x = 0; x < iters; ++x) {
+    const uint32_t i = (uint32_t)x * 32u + (uint32_t)lane;
+    bool mover = false;
+    double4 a = make_double4(0, 0, 0, 0), b = a;
+    if (i < n) {
+      const double4* r = reinterpret_cast<const double4*>(base + (size_t)i * kRecDoubles);
+      a = r[0];
+      const uint32_t dest = tile_of(P, T.tiles_i, T.tiles_j, a.x, a.y, a.z);
+      mover = dest != t;
+      if (mover) {
+        b = r[1];
+        b.w = __longlong_as_double((long long)dest);   // slot 7: destination tile
+      }
+    }
+    const unsigned ball = __ballot_sync(kFull, mover);
+    if (ball) {
+      uint32_t first = 0;
+      if (lane == 0) first = atomicAdd(mv_count, (uint32_t)__popc(ball));
+      first = __shfl_sync(kFull, first, 0);
+      const uint32_t mine = first + (uint32_t)__popc(ball & ((1u << lane) - 1u));
+      if (mover) {
+        if (mine < mv_cap) {
+          double4* o = reinterpret_cast<double4*>(movers + (size_t)mine * kRecDoubles);
+          o[0] = a;
+          o[1] = b;
+          gone |= 1ull << x;
+          ++n_gone;
+        } else {
+          ++n_kept_back;   // mover buffer full: the marker stays (mis-binned) until the next rebin
+        }
+      }
+    }
+  }
+  uint32_t tot_gone = n_gone, tot_back = n_kept_back;
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) {
+    tot_gone += __shfl_xor_sync(kFull, tot_gone, o);
+    tot_back += __shfl_xor_sync(kFull, tot_back, o);
+  }
+  if (tot_gone == 0) {
+    if (lane == 0) {
+      count[t] = n;
+      if (tot_back) atomicAdd(counters + 1, (unsigned long long)tot_back);
+    }
+    return;
+  }
+  const uint32_t n_new = n - tot_gone;
+  // pass 2: holes below n_new, stayers at or above n_new; equally many of both
+  uint32_t nh = 0, nt = 0;
+  for (int x = 0; x < iters; ++x) {
+    const uint32_t i = (uint32_t)x * 32u + (uint32_t)lane;
+    const bool is_gone = (gone >> x) & 1ull;
+    const bool h = i < n_new && is_gone;
+    const bool s = i >= n_new && i < n && !is_gone;
+    const unsigned bh = __ballot_sync(kFull, h), bs = __ballot_sync(kFull, s);
+    if (h) hole[wid][nh + __popc(bh & ((1u << lane) - 1u))] = (unsigned short)i;
+    if (s) tail[wid][nt + __popc(bs & ((1u << lane) - 1u))] = (unsigned short)i;
+    nh += __popc(bh);
+    nt += __popc(bs);
+  }
+  __syncwarp();
+  for (uint32_t q = lane; q < nh; q += 32) {
+    const double4* src = reinterpret_cast<const double4*>(base + (size_t)tail[wid][q] * kRecDoubles);
+    double4* dst = reinterpret_cast<double4*>(base + (size_t)hole[wid][q] * kRecDoubles);
+    const double4 a = src[0], b = src[1];
+    dst[0] = a;
+    dst[1] = b;
+  }
+  if (lane == 0) {
+    count[t] = n_new;
+    atomicAdd(counters, (unsigned long long)tot_gone);
+    if (tot_back) atomicAdd(counters + 1, (unsigned long long)tot_back);
+  }
+}
+
+__global__ void __launch_bounds__(256)
+k_tilebin_insert(const TileBins T, uint32_t* __restrict__ count, double* __restrict__ rec,
+                 const double* __restrict__ movers, uint32_t mv_cap, const uint32_t* __restrict__ mv_count) {
+  const uint32_t n = min(*mv_count, mv_cap);
+  for (uint32_t i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x) {
+    const double4* m = reinterpret_cast<const double4*>(movers + (size_t)i * kRecDoubles);
+    const double4 a = m[0];
+    double4 b = m[1];
+    const uint32_t dest = (uint32_t)__double_as_longlong(b.w);
+    b.w = 0.0;
+    const int64_t dst = claim_slot(count, dest, T.n_tiles, T.cap);
+    if (dst < 0) continue;
+    double4* o = reinterpret_cast<double4*>(rec + dst * kRecDoubles);
+    o[0] = a;
+    o[1] = b;
+  }
+}
+
+}  // namespace
+
+int launch_tilebin_build(const Params& P, const Markers& M, const TileBins& T, uint32_t* count, double* rec,
+                         cudaStream_t st) {
+  if (cudaMemsetAsync(count, 0, (size_t)T.n_tiles * sizeof(uint32_t), st) != cudaSuccess) return -1;
+  if (M.n == 0) return 0;
+  const int64_t blocks = (M.n + 255) / 256;
+  k_tilebin_build<<<(unsigned int)blocks, 256, 0, st>>>(P, M, T, count, rec);
+  return 1;
+}
+
+int launch_tilebin_refresh(const Markers& M, const TileBins& T, const uint32_t* count, double* rec,
+                           cudaStream_t st) {
+  if (M.n == 0) return 0;
+  k_tilebin_refresh<<<T.n_tiles, 128, 0, st>>>(M, T, count, rec);
+  return 1;
+}
+
+int launch_tilebin_rebin(const Params& P, const TileBins& T, uint32_t* count, double* rec, double* movers,
+                         uint32_t mv_cap, uint32_t* mv_count, unsigned long long* counters,
+                         cudaStream_t st) {
+  if (T.cap > 32u * kMaxIter) return -1;
+  if (cudaMemsetAsync(mv_count, 0, sizeof(uint32_t), st) != cudaSuccess) return -1;
+  const unsigned int blocks = (T.n_tiles + kWarpsPerBlock - 1) / kWarpsPerBlock;
+  k_tilebin_extract<<<blocks, kWarpsPerBlock * 32, 0, st>>>(P, T, count, rec, movers, mv_cap, mv_count,
+                                                          counters);
+  unsigned int ib = (mv_cap + 255) / 256;
+  if (ib > 148u * 16u) ib = 148u * 16u;
+  if (ib == 0) ib = 1;
+  k_tilebin_insert<<<ib, 256, 0, st>>>(T, count, rec, movers, mv_cap, mv_count);
+  return 2;
+}
+
+}  // namespace orb

@@ -81,6 +81,23 @@ CONFIGS = {
 }
 
 
+# the paper's single-node workload: 512 x 1024 x 4
+# cells, two kinetic species of 20e6 markers each -- deuterium with adaptive N_L and "heavy"
+# electrons (m_i / m_e = 200).  What the paper does not print is read as follows (R21):
+# rho*_i = 1/720, so that the thermal ion ring spans the same 0.71 radial cells as in cfg1-cfg4;
+# equal temperatures, so rho*_e = rho*_i / sqrt(200); electrons are deposited drift-kinetically
+# (N_L = 1: their ring is 0.05 cells wide); q_e = -1; species s uses seed s.  Both species add into
+# the same rho / j_par (one handle per species: rho* and q belong to the grid descriptor).
+CONFIGS["sn_ion"] = Config("sn_ion", 512, 1024, 4, 20_000_000, 1 / 720, current=True,
+                           adaptive=True, n_max=32)
+CONFIGS["sn_ele"] = Config("sn_ele", 512, 1024, 4, 20_000_000, 1 / (720 * math.sqrt(200.0)),
+                           current=True, n_fixed=1, q=-1.0, seed=1)
+
+# workload name -> the configs (species) deposited into the same grids in one step
+WORKLOADS = {name: (name,) for name in CONFIGS}
+WORKLOADS["single_node"] = ("sn_ion", "sn_ele")
+
+
 def scaled(cfg: Config, n_markers: int, name: str | None = None) -> Config:
     """Same grid/policy, fewer markers (parity cases the oracle finishes quickly)."""
     return dataclasses.replace(cfg, n_markers=n_markers, name=name or f"{cfg.name}@{n_markers}")

@@ -216,3 +216,40 @@ def test_gather_full_size_sampled_markers(name):
     assert np.abs(got - want).max() <= TOL * np.abs(want).max()
     _, npts_o = O.nl_histogram(oracle_geom(cfg), oracle_policy(cfg), m["s"], m["theta"], m["mu"])
     assert npts == npts_o
+
+
+def test_single_node_two_species_workload():
+    """SURVEY 8(f) NEXT-4, the paper's single-node case: 512 x 1024 x 4 cells,
+    deuterium (adaptive N_L) and heavy electrons (N_L = 1, q = -1) of 20e6 markers each, both
+    added into the same rho / j_par.  N_phi = 4: every point touches all four toroidal node
+    planes through the periodic wrap.  Whole grid against the oracle."""
+    import torch
+    cfgs = [W.CONFIGS[n] for n in W.WORKLOADS["single_node"]]
+    shape = (cfgs[0].ns + 3, cfgs[0].ntheta, cfgs[0].nphi)
+    rho = torch.full(shape, 5.0, dtype=torch.float64, device="cuda")
+    jpar = torch.full(shape, -1.0, dtype=torch.float64, device="cuda")
+    st = torch.cuda.current_stream().cuda_stream
+    rho_o, jpar_o = np.zeros(shape), np.zeros(shape)
+    w_sum = 0.0
+    for i, cfg in enumerate(cfgs):
+        m = W.generate(cfg)
+        d = {f: torch.from_numpy(m[f]).cuda() for f in W.FIELDS}
+        g = B.grid_for(cfg)
+        g.markers_bind(d["s"], d["theta"], d["phi"], d["vpar"], d["mu"], d["w"])
+        g.markers_bin(st)
+        if i == 0:
+            g.grid_zero(rho, jpar, st)
+        g.deposit(rho, jpar, B.policy_for(cfg), st)
+        torch.cuda.synchronize()
+        npts, fallback = g.last_points(), g.last_fallback_points()
+        g.destroy()
+        r, j, npts_o, _ = O.deposit_ranges(oracle_geom(cfg), oracle_policy(cfg),
+                                           *(m[f] for f in W.FIELDS), current=True)
+        rho_o += r
+        jpar_o += j
+        w_sum += cfg.q * m["w"].sum()
+        assert npts == npts_o
+        assert fallback < 0.02 * npts
+    assert rel_err(rho.cpu().numpy(), rho_o) <= TOL
+    assert rel_err(jpar.cpu().numpy(), jpar_o) <= TOL
+    assert abs(float(rho.sum().item()) - w_sum) <= 1e-11 * 2e7 * 1e-3

@@ -17,8 +17,9 @@ pytestmark = pytest.mark.gpu
 ALGOS = {
     "atomic": B.ORB_DEPOSIT_ALGO_ATOMIC,
     "atomic_nobin": B.ORB_DEPOSIT_ALGO_ATOMIC | B.ORB_DEPOSIT_NO_BIN,
-    "tile_v4": B.ORB_DEPOSIT_ALGO_TILE_V4,
-    "tile": 0,          # the product path: persistent warp-specialised tile kernel (v5)
+    "tile_v4": B.ORB_DEPOSIT_ALGO_TILE_V4,       # one block per tile
+    "tile_ws": B.ORB_DEPOSIT_ALGO_TILE_WS,       # persistent, warp-specialised
+    "tile": 0,          # the product path: the library picks between the two by N_L policy
 }
 
 
@@ -189,7 +190,7 @@ def test_sorted_flag_on_unsorted_markers_stays_correct(oracle_results):
     result must still be the oracle's (sorted == unsorted)."""
     for name in ("cfg3_small", "cfg4_small"):
         cfg, m, (rho_o, jpar_o, npts_o) = get_case(name, oracle_results)
-        for algo in ("tile", "tile_v4"):
+        for algo in ("tile_ws", "tile_v4"):
             rho, jpar, npts = run_gpu(cfg, m, flags=ALGOS[algo], bind_flags=B.ORB_MARKERS_SORTED)
             assert npts == npts_o
             assert_parity(rho, rho_o, "%s/%s rho" % (name, algo))
