@@ -114,10 +114,11 @@ typedef struct {
                                    binning then only locates the cell boundaries            */
 
 #define ORB_MARKERS_TILE_BINS 0x2u /* bin into slack tile bins (one fixed-capacity segment of records
-                                     per 8 x 16-cell tile and toroidal slab, ~2x the dense layout's
-                                     memory) so that the binning can be refreshed incrementally
-                                     with orb_markers_rebin.  Excludes
-                                     ORB_MARKERS_SORTED.  At most ~1600 markers per tile on average. */
+                                     per 2 x 16 cells and toroidal slab -- a quarter of a deposit
+                                     tile; ~2-3x the dense layout's memory) so that the binning
+                                     can be refreshed incrementally with orb_markers_rebin
+                                     (PAPER.md:235).  Excludes ORB_MARKERS_SORTED.  At most ~1600
+                                     markers per bin on average. */
 
 /* Creates a handle for one grid on desc->device and allocates nothing that
  * scales with the marker count yet.  *out is written only on success. */
@@ -201,7 +202,7 @@ int orb_gather(orb_grid_t *g, int32_t n_fields, const double *const *fields, dou
 /* records <- current values of the bound arrays (every marker; 64-byte record writes). */
 int orb_markers_refresh(orb_grid_t *g, void *stream);
 
-/* Re-derives every record's tile from its (s, theta*, phi); moves the records that left their tile
+/* Re-derives every record's bin from its (s, theta*, phi); moves the records that left their bin
  * (one 32-byte read per marker + 256 bytes per mover).  ORB_E_STATE unless the markers are bound with
  * ORB_MARKERS_TILE_BINS and binned. */
 int orb_markers_rebin(orb_grid_t *g, void *stream);
@@ -211,14 +212,15 @@ int orb_markers_rebin(orb_grid_t *g, void *stream);
 int orb_last_moved(orb_grid_t *g, int64_t *n_moved, int64_t *n_left_in_place);
 
 /* Where the binned records live, for a pusher that updates them in place (DEVICE pointers, owned by
- * the library, valid until the next bind/destroy): record r of tile t is records[(t*capacity + r) *
+ * the library, valid until the next bind/destroy): record r of bin b is records[(b*capacity + r) *
  * record_doubles + {0: s, 1: theta*, 2: phi, 3: vpar, 4: mu, 5: w, 6: index in bound order (int64
- * bits), 7: 0}], r < min(count[t], capacity); tile t = (k_phi*tiles_s + i_s/8)*tiles_theta + j_theta/16. */
+ * bits), 7: 0}], r < min(count[b], capacity);
+ * bin b = ((k_phi*tiles_s + i_s/8)*tiles_theta + j_theta/16)*4 + (i_s%8)/2, n_bins of them. */
 typedef struct {
   double *records;
   const uint32_t *count;
   int32_t record_doubles;
-  uint32_t capacity, n_tiles;
+  uint32_t capacity, n_bins;
   int32_t tiles_s, tiles_theta;
 } orb_marker_layout_t;
 int orb_markers_layout(const orb_grid_t *g, orb_marker_layout_t *out);
@@ -279,8 +281,8 @@ int orb_debug_counters(orb_grid_t *g, uint64_t out[16]);
 int orb_debug_binned(orb_grid_t *g, double *rec_host, uint32_t *cell_start_host,
                      int32_t *rec_doubles);
 
-/* Diagnostic, slack tile bins: count_host (n_tiles uint32) and the records of all tiles, tile by
- * tile, packed into rec_host (n * 8 doubles).  Meant for small cases (one copy per tile). */
+/* Diagnostic, slack tile bins: count_host (n_bins uint32) and the records of all bins, bin by
+ * bin, packed into rec_host (n * 8 doubles).  Meant for small cases (one copy per bin). */
 int orb_debug_tilebins(orb_grid_t *g, double *rec_host, uint32_t *count_host);
 
 /* Host-only diagnostic, no device needed: the polynomial pieces of the clamped (open knot

@@ -50,7 +50,7 @@ class NlPolicy(C.Structure):
 
 class MarkerLayout(C.Structure):
     _fields_ = [("records", C.c_void_p), ("count", C.c_void_p), ("record_doubles", C.c_int32),
-                ("capacity", C.c_uint32), ("n_tiles", C.c_uint32), ("tiles_s", C.c_int32),
+                ("capacity", C.c_uint32), ("n_bins", C.c_uint32), ("tiles_s", C.c_int32),
                 ("tiles_theta", C.c_int32)]
 
 
@@ -188,7 +188,7 @@ class Grid:
         """-> (records (n, 8) packed tile by tile, count per tile)."""
         import numpy as np
         lay = self.markers_layout()
-        cnt = np.empty(lay.n_tiles, dtype=np.uint32)
+        cnt = np.empty(lay.n_bins, dtype=np.uint32)
         rec = np.zeros((n, 8), dtype=np.float64)
         _check(lib().orb_debug_tilebins(self._h, rec.ctypes.data, cnt.ctypes.data), self._h)
         return rec, cnt

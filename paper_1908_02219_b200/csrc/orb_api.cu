@@ -199,14 +199,14 @@ int ensure_tilebins(orb_grid* g, int64_t n) {
   TileBins T;
   T.tiles_i = (g->desc.ns + 7) / 8;
   T.tiles_j = (g->desc.ntheta + 15) / 16;
-  const int64_t n_tiles = (int64_t)T.tiles_i * T.tiles_j * g->desc.nphi;
+  const int64_t n_tiles = (int64_t)T.tiles_i * T.tiles_j * g->desc.nphi * kTileBinSubs;   // bins
   if (n_tiles >= ((int64_t)1 << 31)) return fail(g, ORB_E_INVAL, "too many tiles");
   T.n_tiles = (uint32_t)n_tiles;
   const int64_t mean = (n + n_tiles - 1) / n_tiles;
   int64_t cap = (2 * mean + 128 + 7) & ~(int64_t)7;
   if (cap > 2048) cap = 2048;   // one warp compacts a tile with a 64-bit mask per lane
   if (mean + mean / 4 > cap)
-    return fail(g, ORB_E_INVAL, "ORB_MARKERS_TILE_BINS: more than 1638 markers per tile on average");
+    return fail(g, ORB_E_INVAL, "ORB_MARKERS_TILE_BINS: more than 1638 markers per bin (quarter tile) on average");
   if (n_tiles * cap >= ((int64_t)1 << 32)) return fail(g, ORB_E_INVAL, "tile bins exceed 2^32 records");
   T.cap = (uint32_t)cap;
   T.count = nullptr;
@@ -649,7 +649,7 @@ int orb_markers_layout(const orb_grid_t* g, orb_marker_layout_t* out) {
   out->count = g->tb_count;
   out->record_doubles = kRecDoubles;
   out->capacity = g->tb.cap;
-  out->n_tiles = g->tb.n_tiles;
+  out->n_bins = g->tb.n_tiles;
   out->tiles_s = g->tb.tiles_i;
   out->tiles_theta = g->tb.tiles_j;
   return ORB_OK;

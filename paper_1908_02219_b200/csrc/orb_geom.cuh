@@ -238,18 +238,19 @@ __device__ __forceinline__ MarkerData load_marker(const Markers& M, int64_t p) {
 
 // The markers of grid tile (tj, ti, k) (8 radial x 16 poloidal cells of toroidal slab k), as up to
 // 8 runs of binned records: run r = radial row r of the tile in the dense cell-sorted layout
-// (orb_bin.cu: one contiguous run per row), or the tile's whole segment as run 0 in the slack-tile
-// layout (orb_tilebin.cu).  -> first record and number of records of run r.
+// (orb_bin.cu: one contiguous run per row), or the tile's kTileBinSubs bins as runs 0.. in the
+// slack-tile layout (orb_tilebin.cu).  -> first record and number of records of run r.
 __device__ __forceinline__ void tile_run(const Params& P, const uint32_t* __restrict__ cell_start,
                                          const TileBins& TB, int tj, int ti, int k, int r, uint32_t& b,
                                          uint32_t& n) {
   b = 0;
   n = 0;
   if (TB.count) {
-    if (r == 0) {
+    if (r < kTileBinSubs) {
       const uint32_t t = ((uint32_t)k * (uint32_t)TB.tiles_i + (uint32_t)ti) * (uint32_t)TB.tiles_j + (uint32_t)tj;
-      b = t * TB.cap;
-      n = min(__ldg(TB.count + t), TB.cap);
+      const uint32_t bin = t * (uint32_t)kTileBinSubs + (uint32_t)r;
+      b = bin * TB.cap;
+      n = min(__ldg(TB.count + bin), TB.cap);
     }
     return;
   }

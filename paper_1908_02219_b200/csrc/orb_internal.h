@@ -54,12 +54,14 @@ struct Markers {
   int64_t n;
 };
 
-// Slack tile bins (orb_tilebin.cu, NEXT-2): tile t = (k * tiles_i + ti) * tiles_j + tj owns the records
-// [t * cap, t * cap + min(count[t], cap)) of Markers::rec.  count == nullptr: the dense cell-sorted
+// Slack tile bins (orb_tilebin.cu, NEXT-2): tile t = (k * tiles_i + ti) * tiles_j + tj is cut into
+// kTileBinSubs bins of 8 / kTileBinSubs radial rows; bin b = t * kTileBinSubs + sub owns the records
+// [b * cap, b * cap + min(count[b], cap)) of Markers::rec.  count == nullptr: the dense cell-sorted
 // layout of orb_bin.cu (per-cell offsets) is in use instead.
+constexpr int kTileBinSubs = 4;
 struct TileBins {
   const uint32_t* count;
-  uint32_t cap, n_tiles;
+  uint32_t cap, n_tiles;   // n_tiles: number of BINS (tiles * kTileBinSubs)
   int tiles_i, tiles_j;
 };
 

@@ -4,14 +4,17 @@
 // cannot be updated in place (any insertion shifts everything behind it), so this second binning
 // layout trades memory for updatability:
 //
-//   slack tile bins   the grid's deposit tiles (1 toroidal slab x 8 radial x 16 poloidal cells,
-//                     the unit of work of the tile kernels) each own a fixed-capacity segment
-//                     rec[t * cap .. t * cap + count[t]) of 64-byte marker records, in any order
-//                     (the tile kernels sort a tile's Larmor points on chip anyway, so per-cell
-//                     order inside a tile buys nothing).  cap ~ 2 x the mean occupancy + 128.
+//   slack tile bins   every deposit tile (1 toroidal slab x 8 radial x 16 poloidal cells, the unit
+//                     of work of the tile kernels) is cut into 4 bins of 2 radial rows; bin b owns
+//                     a fixed-capacity segment rec[b * cap .. b * cap + count[b]) of 64-byte marker
+//                     records, in any order.  (Whole-tile bins were measured first: the tile
+//                     kernels take a tile's markers in chunks of 256-384, and a chunk drawn from
+//                     the whole tile spreads its Larmor points over all 288 cells of the halo
+//                     window -- 1.9x slower deposits than chunks of 2-4 radial rows.)
+//                     cap ~ 2 x the mean occupancy + 128.
 //   build             ONE pass: slot = atomicAdd(count[tile]); no histogram, no scan.
 //   rebin             after the marker coordinates changed in the records (orb_markers_refresh,
-//                     or a pusher writing them in place): one warp per tile re-derives each
+//                     or a pusher writing them in place): one warp per bin re-derives each
 //                     record's tile; markers that left are copied to a mover buffer and the
 //                     segment is compacted (tail records fill the holes); a second kernel
 //                     appends the movers to their new tiles.  Cost: one 32-byte sector per marker
@@ -37,8 +40,9 @@ __device__ __forceinline__ uint32_t tile_of(const Params& P, int tiles_i, int ti
   int k = (int)(wrap_2pi(ph) * P.nph_scale);
   j = min(max(j, 0), P.nth - 1);
   k = min(max(k, 0), P.nph - 1);
-  return ((uint32_t)k * (uint32_t)tiles_i + (uint32_t)(i / kTileI)) * (uint32_t)tiles_j +
-         (uint32_t)(j / kTileJ);
+  const uint32_t tile = ((uint32_t)k * (uint32_t)tiles_i + (uint32_t)(i / kTileI)) * (uint32_t)tiles_j +
+                        (uint32_t)(j / kTileJ);
+  return tile * (uint32_t)kTileBinSubs + (uint32_t)((i % kTileI) / (kTileI / kTileBinSubs));
 }
 
 // claim a slot in tile t, or in the next tile with room (benign mis-binning, see the header)
@@ -89,10 +93,12 @@ k_tilebin_refresh(const Markers M, const TileBins T, const uint32_t* __restrict_
   }
 }
 
-// One warp per tile: movers out, segment compacted.  counters[0] += movers extracted,
-// counters[1] += movers left in place because the mover buffer was full.
-constexpr int kWarpsPerBlock = 4;
-constexpr int kMaxIter = 64;    // cap <= 32 * kMaxIter records per tile
+// One warp per bin: movers out, segment compacted.  counters[0] += movers extracted,
+// counters[1] += movers left in place because the mover buffer was full.  The mover buffer is
+// claimed once per BLOCK (one atomic on the shared counter per 8 bins, not per warp pass: with a
+// counter per pass the kernel was bound by same-address atomics, 1.4 ms at 1 % movers on cfg3).
+constexpr int kWarpsPerBlock = 8;
+constexpr int kMaxIter = 64;    // cap <= 32 * kMaxIter records per bin
 
 __global__ void __launch_bounds__(kWarpsPerBlock * 32)
 k_tilebin_extract(const Params P, const TileBins T, uint32_t* __restrict__ count, double* __restrict__ rec,
@@ -100,64 +106,77 @@ k_tilebin_extract(const Params P, const TileBins T, uint32_t* __restrict__ count
                   unsigned long long* __restrict__ counters) {
   __shared__ unsigned short hole[kWarpsPerBlock][32 * kMaxIter / 2 + 32];
   __shared__ unsigned short tail[kWarpsPerBlock][32 * kMaxIter / 2 + 32];
+  __shared__ uint32_t warp_movers[kWarpsPerBlock];
+  __shared__ uint32_t block_base;
   const int wid = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const uint32_t t = blockIdx.x * kWarpsPerBlock + wid;
-  if (t >= T.n_tiles) return;
-  const uint32_t n = min(count[t], T.cap);
-  if (n == 0) {
-    if (lane == 0) count[t] = 0;
-    return;
-  }
-  double* base = rec + (int64_t)t * T.cap * kRecDoubles;
+  const bool live = t < T.n_tiles;
+  const uint32_t n = live ? min(count[t], T.cap) : 0u;
+  double* base = rec + (int64_t)(live ? t : 0) * T.cap * kRecDoubles;
   const int iters = (int)((n + 31) / 32);
-  // pass 1: who leaves?  bit x of `gone`: record x * 32 + lane is a mover that was copied out
+  // pass 1: who leaves?  bit x of `gone`: record x * 32 + lane belongs to another bin
   unsigned long long gone = 0;
-  uint32_t n_gone = 0, n_kept_back = 0;
+  uint32_t n_gone = 0;
   for (int x = 0; x < iters; ++x) {
     const uint32_t i = (uint32_t)x * 32u + (uint32_t)lane;
-    bool mover = false;
-    double4 a = make_double4(0, 0, 0, 0), b = a;
     if (i < n) {
-      const double4* r = reinterpret_cast<const double4*>(base + (size_t)i * kRecDoubles);
-      a = r[0];
-      const uint32_t dest = tile_of(P, T.tiles_i, T.tiles_j, a.x, a.y, a.z);
-      mover = dest != t;
-      if (mover) {
-        b = r[1];
-        b.w = __longlong_as_double((long long)dest);   // slot 7: destination tile
-      }
-    }
-    const unsigned ball = __ballot_sync(kFull, mover);
-    if (ball) {
-      uint32_t first = 0;
-      if (lane == 0) first = atomicAdd(mv_count, (uint32_t)__popc(ball));
-      first = __shfl_sync(kFull, first, 0);
-      const uint32_t mine = first + (uint32_t)__popc(ball & ((1u << lane) - 1u));
-      if (mover) {
-        if (mine < mv_cap) {
-          double4* o = reinterpret_cast<double4*>(movers + (size_t)mine * kRecDoubles);
-          o[0] = a;
-          o[1] = b;
-          gone |= 1ull << x;
-          ++n_gone;
-        } else {
-          ++n_kept_back;   // mover buffer full: the marker stays (mis-binned) until the next rebin
-        }
+      const double4 a = *reinterpret_cast<const double4*>(base + (size_t)i * kRecDoubles);
+      if (tile_of(P, T.tiles_i, T.tiles_j, a.x, a.y, a.z) != t) {
+        gone |= 1ull << x;
+        ++n_gone;
       }
     }
   }
-  uint32_t tot_gone = n_gone, tot_back = n_kept_back;
+  uint32_t incl = n_gone;   // inclusive prefix over the lanes
+#pragma unroll
+  for (int o = 1; o < 32; o <<= 1) {
+    const uint32_t v = __shfl_up_sync(kFull, incl, o);
+    if (lane >= o) incl += v;
+  }
+  const uint32_t warp_total = __shfl_sync(kFull, incl, 31);
+  if (lane == 0) warp_movers[wid] = warp_total;
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    uint32_t tot = 0;
+    for (int w = 0; w < kWarpsPerBlock; ++w) tot += warp_movers[w];
+    block_base = tot ? atomicAdd(mv_count, tot) : 0u;
+  }
+  __syncthreads();
+  if (!live || n == 0) {
+    if (live && lane == 0) count[t] = 0;
+    return;
+  }
+  if (warp_total == 0) {
+    if (lane == 0) count[t] = n;
+    return;
+  }
+  uint32_t my_slot = block_base + (incl - n_gone);
+  for (int w = 0; w < wid; ++w) my_slot += warp_movers[w];
+  // pass 1b: copy this lane's movers out (slot 7 <- destination bin); movers beyond the buffer's
+  // capacity stay where they are (mis-binned) until the next rebin
+  uint32_t n_back = 0;
+  for (int x = 0; x < iters; ++x) {
+    if (!((gone >> x) & 1ull)) continue;
+    if (my_slot < mv_cap) {
+      const uint32_t i = (uint32_t)x * 32u + (uint32_t)lane;
+      const double4* r = reinterpret_cast<const double4*>(base + (size_t)i * kRecDoubles);
+      const double4 a = r[0];
+      double4 b = r[1];
+      b.w = __longlong_as_double((long long)tile_of(P, T.tiles_i, T.tiles_j, a.x, a.y, a.z));
+      double4* o = reinterpret_cast<double4*>(movers + (size_t)my_slot * kRecDoubles);
+      o[0] = a;
+      o[1] = b;
+    } else {
+      gone &= ~(1ull << x);
+      ++n_back;
+    }
+    ++my_slot;
+  }
+  uint32_t tot_gone = n_gone - n_back, tot_back = n_back;
 #pragma unroll
   for (int o = 16; o > 0; o >>= 1) {
     tot_gone += __shfl_xor_sync(kFull, tot_gone, o);
     tot_back += __shfl_xor_sync(kFull, tot_back, o);
-  }
-  if (tot_gone == 0) {
-    if (lane == 0) {
-      count[t] = n;
-      if (tot_back) atomicAdd(counters + 1, (unsigned long long)tot_back);
-    }
-    return;
   }
   const uint32_t n_new = n - tot_gone;
   // pass 2: holes below n_new, stayers at or above n_new; equally many of both
@@ -183,7 +202,7 @@ k_tilebin_extract(const Params P, const TileBins T, uint32_t* __restrict__ count
   }
   if (lane == 0) {
     count[t] = n_new;
-    atomicAdd(counters, (unsigned long long)tot_gone);
+    if (tot_gone) atomicAdd(counters, (unsigned long long)tot_gone);
     if (tot_back) atomicAdd(counters + 1, (unsigned long long)tot_back);
   }
 }
