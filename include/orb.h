@@ -94,6 +94,13 @@ enum { ORB_NL_FIXED = 0, ORB_NL_ADAPTIVE = 1 };
                                         kernels by N_L policy: persistent for fixed N_L <= 4,
                                         one-block-per-tile for larger or adaptive N_L.            */
 
+#define ORB_DEPOSIT_ALGO_RING_DATA 0x20u /* the paper's own organisation, as a
+                                        measured alternative: materialise the Larmor ring data in
+                                        device memory, bucket-sort the Larmor POINTS by field
+                                        cell, then loop over cells with the points of a cell in
+                                        the inner loop.  Needs orb_ring_reserve; uses the bound
+                                        arrays directly (no marker binning).                     */
+
 /* Number of Larmor points per marker (R7-R9):
  *   FIXED:    N_L = n_fixed
  *   ADAPTIVE: N_L = min(n_max, n_fixed * max(1, ceil(rho_L / rho_ref)))
@@ -149,6 +156,12 @@ int orb_markers_bind(orb_grid_t *g, int64_t n, const double *s, const double *th
 /* Pre-allocates the marker-proportional scratch for up to n markers (ORB_E_NOMEM if the
  * device cannot hold it).  Optional: orb_markers_bind grows it on demand. */
 int orb_reserve(orb_grid_t *g, int64_t n);
+
+/* Reserves the scratch of ORB_DEPOSIT_ALGO_RING_DATA: Larmor ring data for up to n_points Larmor
+ * points (2 x 48 bytes each: in marker order and sorted by cell) of up to n_markers markers.
+ * Allocates (synchronises); call it outside timed / captured regions.  Points beyond n_points are
+ * still deposited (directly, with global atomics) and counted by orb_last_fallback_points. */
+int orb_ring_reserve(orb_grid_t *g, int64_t n_markers, int64_t n_points);
 
 /* Runs (or refreshes) the binning pass alone on `stream`, so that it can be timed
  * apart from the deposit (BASELINE.json config 4; the bucket sort of PAPER.md:167):

@@ -18,6 +18,7 @@ ORB_DEPOSIT_NO_BIN = 0x2
 ORB_DEPOSIT_ALGO_ATOMIC = 0x4
 ORB_DEPOSIT_ALGO_TILE_V4 = 0x8
 ORB_DEPOSIT_ALGO_TILE_WS = 0x10
+ORB_DEPOSIT_ALGO_RING_DATA = 0x20
 ORB_MARKERS_SORTED = 0x1
 ORB_MARKERS_TILE_BINS = 0x2
 ORB_MAX_NL = 32
@@ -25,7 +26,7 @@ ORB_MAX_FIELDS = 8
 
 # every symbol include/orb.h declares
 SYMBOLS = ("orb_grid_create", "orb_grid_destroy", "orb_grid_shape", "orb_markers_bind",
-           "orb_reserve", "orb_markers_bin", "orb_markers_refresh", "orb_markers_rebin", "orb_last_moved",
+           "orb_reserve", "orb_ring_reserve", "orb_markers_bin", "orb_markers_refresh", "orb_markers_rebin", "orb_last_moved",
            "orb_markers_layout", "orb_debug_tilebins", "orb_deposit", "orb_gather", "orb_grid_zero", "orb_last_points", "orb_last_fallback_points", "orb_deposit_host",
            "orb_launch_count", "orb_debug_counters", "orb_debug_binned", "orb_probe_dfma", "orb_spline_table_radial", "orb_strerror", "orb_last_error", "orb_version")
 
@@ -72,6 +73,7 @@ def lib():
     L.orb_grid_shape.argtypes = [vp, C.POINTER(C.c_int64 * 3)]
     L.orb_markers_bind.argtypes = [vp, C.c_int64, dp, dp, dp, dp, dp, dp, C.c_uint32]
     L.orb_reserve.argtypes = [vp, C.c_int64]
+    L.orb_ring_reserve.argtypes = [vp, C.c_int64, C.c_int64]
     L.orb_markers_bin.argtypes = [vp, vp]
     L.orb_markers_refresh.argtypes = [vp, vp]
     L.orb_markers_rebin.argtypes = [vp, vp]
@@ -163,6 +165,9 @@ class Grid:
 
     def reserve(self, n):
         _check(lib().orb_reserve(self._h, n), self._h)
+
+    def ring_reserve(self, n_markers, n_points):
+        _check(lib().orb_ring_reserve(self._h, n_markers, n_points), self._h)
 
     def markers_bin(self, stream=None):
         _check(lib().orb_markers_bin(self._h, stream), self._h)

@@ -50,6 +50,8 @@ struct orb_grid {
   uint32_t* tb_mv_count;
   unsigned long long* tb_counters;   // [0] movers of the last rebin, [1] movers left in place
 
+  RingScratch ringdata;      // Larmor ring data (orb_ring_reserve; orb_cellowner.cu), owned
+
   // orb_deposit_host staging (owned)
   double* hbuf[6];
   int64_t hbuf_capacity;
@@ -178,6 +180,15 @@ int ensure_bin_scratch(orb_grid* g, int64_t n) {
     g->bin_capacity = n;
   }
   return ORB_OK;
+}
+
+void free_ringdata(orb_grid* g) {
+  cudaFree(g->ringdata.off);
+  cudaFree(g->ringdata.cell_start);
+  cudaFree(g->ringdata.block_sums);
+  cudaFree(g->ringdata.ring);
+  cudaFree(g->ringdata.sorted);
+  memset(&g->ringdata, 0, sizeof(g->ringdata));
 }
 
 void free_tilebins(orb_grid* g) {
@@ -341,6 +352,7 @@ int orb_grid_destroy(orb_grid_t* g) {
   cudaDeviceSynchronize();
   free_bin(g);
   free_tilebins(g);
+  free_ringdata(g);
   cudaFree(g->bin.cell_start);
   cudaFree(g->bin.block_sums);
   cudaFree(g->scoef);
@@ -423,6 +435,34 @@ int orb_reserve(orb_grid_t* g, int64_t n) {
   return ensure_bin_scratch(g, n);
 }
 
+int orb_ring_reserve(orb_grid_t* g, int64_t n_markers, int64_t n_points) {
+  if (!g) return ORB_E_INVAL;
+  if (n_markers < 0 || n_points < 0 || n_markers >= ((int64_t)1 << 32) - 1 ||
+      n_points >= ((int64_t)1 << 32) - 1)
+    return fail(g, ORB_E_INVAL, "orb_ring_reserve: counts out of range");
+  DeviceGuard dg(g->desc.device);
+  if (!dg.ok) return fail(g, ORB_E_CUDA, "cudaSetDevice");
+  if (n_markers <= g->ringdata.markers && n_points <= g->ringdata.capacity) return ORB_OK;
+  free_ringdata(g);
+  RingScratch R;
+  memset(&R, 0, sizeof(R));
+  const int64_t widest = n_markers > g->ncells ? n_markers : g->ncells;
+  const size_t pts = (size_t)(n_points > 0 ? n_points : 1) * 6 * sizeof(double);
+  if (cudaMalloc(&R.off, (size_t)(n_markers + 1) * sizeof(uint32_t)) != cudaSuccess ||
+      cudaMalloc(&R.cell_start, (size_t)(g->ncells + 1) * sizeof(uint32_t)) != cudaSuccess ||
+      cudaMalloc(&R.block_sums, (size_t)(widest / 4096 + 2) * sizeof(uint32_t)) != cudaSuccess ||
+      cudaMalloc(&R.ring, pts) != cudaSuccess || cudaMalloc(&R.sorted, pts) != cudaSuccess) {
+    cudaGetLastError();
+    g->ringdata = R;
+    free_ringdata(g);
+    return fail(g, ORB_E_NOMEM, "Larmor ring data");
+  }
+  R.capacity = n_points;
+  R.markers = n_markers;
+  g->ringdata = R;
+  return ORB_OK;
+}
+
 int orb_markers_bin(orb_grid_t* g, void* stream) {
   if (!g) return ORB_E_INVAL;
   if (!g->have_bind) return fail(g, ORB_E_STATE, "orb_markers_bin before orb_markers_bind");
@@ -447,11 +487,14 @@ int orb_deposit(orb_grid_t* g, double* rho, double* jpar, const orb_nl_policy_t*
 
   rc = upload_ring(g, pol->alpha0, st);
   if (rc != ORB_OK) return rc;
+  const bool ring_algo = (pol->flags & ORB_DEPOSIT_ALGO_RING_DATA) != 0;
+  if (ring_algo && (!g->ringdata.off || g->bound.n > g->ringdata.markers))
+    return fail(g, ORB_E_STATE, "ORB_DEPOSIT_ALGO_RING_DATA needs orb_ring_reserve for the bound markers");
   const bool atomic_algo = (pol->flags & ORB_DEPOSIT_ALGO_ATOMIC) != 0;
   const bool tile_v4 = (pol->flags & ORB_DEPOSIT_ALGO_TILE_V4) != 0;
   const bool tile_v5 = (pol->flags & ORB_DEPOSIT_ALGO_TILE_WS) != 0;
   const bool no_bin = (pol->flags & ORB_DEPOSIT_NO_BIN) != 0;
-  if (!no_bin && !atomic_algo && !g->binned) {
+  if (!no_bin && !atomic_algo && !ring_algo && !g->binned) {
     rc = do_bin(g, st);
     if (rc != ORB_OK) return rc;
   }
@@ -470,7 +513,10 @@ int orb_deposit(orb_grid_t* g, double* rho, double* jpar, const orb_nl_policy_t*
   TileBins TB = g->tb;
   if (!g->tile_mode) TB.count = nullptr;
   int l;
-  if (atomic_algo || !use_binned) {
+  if (ring_algo) {
+    M.rec = nullptr;   // the Larmor ring data are built from the bound arrays; no marker binning
+    l = launch_deposit_ringdata(P, M, g->ringdata, rho, jpar, g->d_points, st);
+  } else if (atomic_algo || !use_binned) {
     l = launch_deposit_atomic(P, M, rho, jpar, g->d_points, st);
   } else if (tile_v4 || (!tile_v5 && (P.adaptive || P.n_fixed > 4))) {
     // N_L > 4 or adaptive: the one-block-per-tile kernel, whose point slots are filled by a

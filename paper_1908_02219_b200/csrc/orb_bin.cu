@@ -143,6 +143,16 @@ k_bin_scatter(const Params P, const Markers M, const uint32_t* __restrict__ cell
                : "memory");
 }
 
+// exclusive scan in place: count[0..n) -> offsets, count[n] = total; block_sums: n / 4096 + 2 words
+int launch_scan(uint32_t* count, int64_t n, uint32_t* block_sums, cudaStream_t st) {
+  const int nb = (int)((n + kScanTile - 1) / kScanTile);
+  if (nb == 0) return 0;
+  k_scan_reduce<<<nb, kScanThreads, 0, st>>>(count, n, block_sums);
+  k_scan_block_sums<<<1, kScanThreads, 0, st>>>(block_sums, nb);
+  k_scan_apply<<<nb, kScanThreads, 0, st>>>(count, n, block_sums);
+  return 3;
+}
+
 int launch_bin(const Params& P, const Markers& M, const BinScratch& B, bool presorted,
                cudaStream_t st) {
   int launches = 0;
@@ -155,11 +165,7 @@ int launch_bin(const Params& P, const Markers& M, const BinScratch& B, bool pres
                                                       presorted ? nullptr : B.rank);
     ++launches;
   }
-  const int nb = (int)((nc + kScanTile - 1) / kScanTile);
-  k_scan_reduce<<<nb, kScanThreads, 0, st>>>(B.cell_start, nc, B.block_sums);
-  k_scan_block_sums<<<1, kScanThreads, 0, st>>>(B.block_sums, nb);
-  k_scan_apply<<<nb, kScanThreads, 0, st>>>(B.cell_start, nc, B.block_sums);
-  launches += 3;
+  launches += launch_scan(B.cell_start, nc, B.block_sums, st);
   if (!presorted && M.n > 0) {
     const int64_t blocks = (M.n + 255) / 256;
     k_bin_scatter<<<(unsigned int)blocks, 256, 0, st>>>(P, M, B.cell_start, B.rank, B.rec);

@@ -38,7 +38,7 @@
 // leaves the tile's halo (long rings, rounding at a slab boundary) are deposited directly with
 // global atomics (rare; counted).
 //
-// Why this shape (profiles/r01_microbench.md, r01_v2_deposit_ncu.md, r01_v4_deposit_ncu.md):
+// Why this shape (profiles/r01_microbench.md, profiles/r01_final_deposit_ncu.md):
 // shared-memory fp64 atomics are CAS loops (1.5 updates/clk/SM) and global fp64 REDs issue at
 // 0.78 lanes/clk/SM, while the path needs 128 node updates per Larmor point; only register
 // accumulators keep up with the fp64 pipe (64 FMA/clk/SM).  DMMA m8n8k4 occupies that pipe for

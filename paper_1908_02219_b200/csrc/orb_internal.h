@@ -103,6 +103,19 @@ int launch_tilebin_rebin(const Params& P, const TileBins& T, uint32_t* count, do
                          uint32_t mv_cap, uint32_t* mv_count, unsigned long long* counters,
                          cudaStream_t st);
 
+// Materialised Larmor ring data + cell-owner deposition (orb_cellowner.cu, NEXT-3)
+struct RingScratch {
+  uint32_t* off;         // markers + 1: N_L per marker -> first point slot of the marker
+  uint32_t* cell_start;  // ncells + 1: Larmor points per cell -> offsets
+  uint32_t* block_sums;  // scan scratch for both
+  double* ring;          // capacity * 6 doubles, marker order
+  double* sorted;        // capacity * 6 doubles, cell order
+  int64_t capacity;      // Larmor points the two arrays hold
+  int64_t markers;       // markers off[] can hold
+};
+int launch_deposit_ringdata(const Params& P, const Markers& M, const RingScratch& R, double* rho,
+                            double* jpar, unsigned long long* d_points, cudaStream_t st);
+
 // ring table (cos, sin)(alpha0 + 2 pi l / N), built on the device (orb_ring.cu)
 int launch_ring_table(double2* ring, double alpha0, cudaStream_t st);
 

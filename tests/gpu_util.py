@@ -35,6 +35,13 @@ def to_device(m):
     return {f: torch.from_numpy(np.ascontiguousarray(m[f])).cuda() for f in W.FIELDS}
 
 
+def prepare(g, cfg, flags):
+    """Scratch an algorithm flag needs before orb_deposit (the ring-data path reserves its Larmor
+    ring data outside the deposit call)."""
+    if flags & B.ORB_DEPOSIT_ALGO_RING_DATA:
+        g.ring_reserve(cfg.n_markers, cfg.n_markers * (cfg.n_max if cfg.adaptive else cfg.n_fixed))
+
+
 def run_gpu(cfg, m, flags=0, bind_flags=0, dev=None, bin_first=False, theta_map=1, repeat=1):
     """One orb_deposit through the C ABI on cuda:0. -> (rho, jpar, n_points) as numpy."""
     import torch
@@ -51,6 +58,7 @@ def run_gpu(cfg, m, flags=0, bind_flags=0, dev=None, bin_first=False, theta_map=
         if bin_first:
             g.markers_bin(st)
         pol = B.policy_for(cfg, flags=flags)
+        prepare(g, cfg, flags)
         for _ in range(repeat):
             g.deposit(rho, jpar, pol, st)
         npts = g.last_points()

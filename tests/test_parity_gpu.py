@@ -9,8 +9,8 @@ import pytest
 from paper_1908_02219_b200 import binding as B
 from paper_1908_02219_b200 import workloads as W
 
-from gpu_util import (assert_parity, oracle_geom, oracle_policy, rel_err, run_gpu, run_oracle,
-                      to_device)
+from gpu_util import (assert_parity, oracle_geom, oracle_policy, prepare, rel_err, run_gpu,
+                      run_oracle, to_device)
 
 pytestmark = pytest.mark.gpu
 
@@ -19,6 +19,7 @@ ALGOS = {
     "atomic_nobin": B.ORB_DEPOSIT_ALGO_ATOMIC | B.ORB_DEPOSIT_NO_BIN,
     "tile_v4": B.ORB_DEPOSIT_ALGO_TILE_V4,       # one block per tile
     "tile_ws": B.ORB_DEPOSIT_ALGO_TILE_WS,       # persistent, warp-specialised
+    "ring_data": B.ORB_DEPOSIT_ALGO_RING_DATA,   # NEXT-3: Larmor ring data + cell-owner loop
     "tile": 0,          # the product path: the library picks between the two by N_L policy
 }
 
@@ -281,6 +282,29 @@ def test_cuda_graph_capture_of_bin_zero_deposit(oracle_results):
         g.destroy()
 
 
+def test_ring_data_capacity_overflow_is_benign(oracle_results):
+    """NEXT-3: Larmor ring data reserved for fewer points than the markers produce -- the points
+    beyond the reservation are deposited directly and counted; the grids still match the oracle."""
+    import torch
+    cfg, m, (rho_o, jpar_o, npts_o) = get_case("cfg4_small", oracle_results)
+    d = to_device(m)
+    g = B.grid_for(cfg)
+    rho = torch.zeros(g.shape(), dtype=torch.float64, device="cuda")
+    jpar = torch.zeros_like(rho)
+    g.markers_bind(d["s"], d["theta"], d["phi"], d["vpar"], d["mu"], d["w"])
+    with pytest.raises(B.OrbError) as e:
+        g.deposit(rho, jpar, B.policy_for(cfg, flags=B.ORB_DEPOSIT_ALGO_RING_DATA))
+    assert e.value.code == B.ORB_E_STATE            # no orb_ring_reserve yet
+    g.ring_reserve(cfg.n_markers, npts_o // 2)
+    g.deposit(rho, jpar, B.policy_for(cfg, flags=B.ORB_DEPOSIT_ALGO_RING_DATA),
+              torch.cuda.current_stream().cuda_stream)
+    assert g.last_points() == npts_o
+    assert g.last_fallback_points() == npts_o - npts_o // 2
+    g.destroy()
+    assert_parity(rho.cpu().numpy(), rho_o)
+    assert_parity(jpar.cpu().numpy(), jpar_o)
+
+
 def test_error_codes():
     import torch
     g = B.Grid(16, 32, 16)
@@ -340,6 +364,7 @@ def test_nondefault_geometry_charge_field_and_gyrophase(adaptive):
         g.markers_bind(d["s"], d["theta"], d["phi"], d["vpar"], d["mu"], d["w"])
         pol = B.policy(cfg.n_fixed, adaptive=adaptive, n_max=cfg.n_max if adaptive else None,
                        rho_ref=cfg.rho_ref, alpha0=alpha0, flags=flags)
+        prepare(g, cfg, flags)
         g.deposit(rho, jpar, pol, torch.cuda.current_stream().cuda_stream)
         npts = g.last_points()
         g.destroy()
