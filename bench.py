@@ -153,7 +153,7 @@ def config_json(cfgs, world, workload=None, extra=None):
     if not isinstance(cfgs, (list, tuple)):
         cfgs = [cfgs]
     c = {"workload": " + ".join(describe(x) for x in cfgs) if len(cfgs) > 1 else describe(cfgs[0]),
-         "step": "per species: bind + bin (counting sort by cell) + tile deposit; grids zeroed once",
+         "step": "per species: bind + bin + tile deposit; grids zeroed once",
          "l2_policy": "inputs (%.2f GB markers) larger than the 126 MB L2; no flush needed"
                       % (sum(x.n_markers for x in cfgs) * 48 / 1e9),
          "parallelism": "replicas x%d (no sharding, no collective)" % world if world > 1 else "1 GPU"}
@@ -217,7 +217,7 @@ def run_reference(args):
 class Species:
     """One marker species of the workload: pinned host arrays, device copies, its grid handle."""
 
-    def __init__(self, cfg, dev, local_rank, B, torch):
+    def __init__(self, cfg, dev, local_rank, B, torch, binning):
         self.cfg = cfg
         n = cfg.n_markers
         self.host = {f: torch.empty(n, dtype=torch.float64, pin_memory=True) for f in W.FIELDS}
@@ -226,7 +226,8 @@ class Species:
         self.d = {f: self.host[f].to(dev, non_blocking=True) for f in W.FIELDS}
         self.g = B.grid_for(cfg, device=local_rank)
         self.pol = B.policy_for(cfg)
-        self.bind_flags = B.ORB_MARKERS_SORTED if cfg.order == "sorted" else 0
+        self.bind_flags = (B.ORB_MARKERS_SORTED if cfg.order == "sorted"
+                           else B.ORB_MARKERS_TILE_BINS if binning == "tile" else 0)
 
     def bind(self):
         d, cfg = self.d, self.cfg
@@ -265,7 +266,7 @@ def run_ours(args):
 
     # inputs: generated on the host into pinned memory (they are the e2e leg's source)
     cfgs = [pick_config(name, rank) for name in W.WORKLOADS[args.workload]]
-    species = [Species(c, dev, local_rank, B, torch) for c in cfgs]
+    species = [Species(c, dev, local_rank, B, torch, args.binning) for c in cfgs]
     torch.cuda.synchronize()
     cfg = cfgs[0]                     # grid shape and outputs are common to the species
     current = any(c.current for c in cfgs)
@@ -418,7 +419,9 @@ def run_ours(args):
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K,
             "warmup": args.warmup, "ms_per_step": job_ms / K, "higher_is_better": True,
             "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-            "config": config_json(cfgs, world, args.workload),
+            "config": config_json(cfgs, world, args.workload, {
+                "binning": "slack tile bins, one pass (ORB_MARKERS_TILE_BINS)" if args.binning == "tile"
+                else "dense counting sort by cell (count, scan, scatter)"}),
             "points_per_step": npts_step,
             "fallback_points_per_step": fallback_step,
             "phases_ms": {"bin": bin_ms, "zero": zero_ms, "deposit": dep_ms,
@@ -493,6 +496,9 @@ def main(argv=None):
     ap.add_argument("--ref-sample", type=int, default=1 << 18,
                     help="markers per step of the --impl reference arm")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--binning", default="tile", choices=["tile", "dense"],
+                    help="marker binning of the step: slack tile bins built in one pass "
+                         "(ORB_MARKERS_TILE_BINS) or the dense counting sort by cell")
     ap.add_argument("--no-gather", action="store_true", help="skip the orb_gather (NEXT-1) leg")
     args = ap.parse_args(argv)
     if args.warmup < 3 and args.impl == "ours":

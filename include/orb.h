@@ -121,11 +121,11 @@ typedef struct {
                                    binning then only locates the cell boundaries            */
 
 #define ORB_MARKERS_TILE_BINS 0x2u /* bin into slack tile bins (one fixed-capacity segment of records
-                                     per 2 x 16 cells and toroidal slab -- a quarter of a deposit
-                                     tile; ~2-3x the dense layout's memory) so that the binning
-                                     can be refreshed incrementally with orb_markers_rebin
-                                     (PAPER.md:235).  Excludes ORB_MARKERS_SORTED.  At most ~1600
-                                     markers per bin on average. */
+                                     per 1 x 16 cells and toroidal slab -- one radial row of a
+                                     deposit tile; ~2.5x the dense layout's memory): built in ONE
+                                     pass (no histogram, no scan) and refreshed incrementally with
+                                     orb_markers_rebin.  Excludes
+                                     ORB_MARKERS_SORTED.  At most ~1300 markers per bin on average. */
 
 /* Creates a handle for one grid on desc->device and allocates nothing that
  * scales with the marker count yet.  *out is written only on success. */
@@ -228,7 +228,7 @@ int orb_last_moved(orb_grid_t *g, int64_t *n_moved, int64_t *n_left_in_place);
  * the library, valid until the next bind/destroy): record r of bin b is records[(b*capacity + r) *
  * record_doubles + {0: s, 1: theta*, 2: phi, 3: vpar, 4: mu, 5: w, 6: index in bound order (int64
  * bits), 7: 0}], r < min(count[b], capacity);
- * bin b = ((k_phi*tiles_s + i_s/8)*tiles_theta + j_theta/16)*4 + (i_s%8)/2, n_bins of them. */
+ * bin b = ((k_phi*tiles_s + i_s/8)*tiles_theta + j_theta/16)*8 + i_s%8, n_bins of them. */
 typedef struct {
   double *records;
   const uint32_t *count;

@@ -214,10 +214,10 @@ int ensure_tilebins(orb_grid* g, int64_t n) {
   if (n_tiles >= ((int64_t)1 << 31)) return fail(g, ORB_E_INVAL, "too many tiles");
   T.n_tiles = (uint32_t)n_tiles;
   const int64_t mean = (n + n_tiles - 1) / n_tiles;
-  int64_t cap = (2 * mean + 128 + 7) & ~(int64_t)7;
-  if (cap > 2048) cap = 2048;   // one warp compacts a tile with a 64-bit mask per lane
+  int64_t cap = (mean + mean / 2 + 64 + 7) & ~(int64_t)7;   // occupied bins hold ~1.25 x the mean
+  if (cap > 2048) cap = 2048;   // one warp compacts a bin with a 64-bit mask per lane
   if (mean + mean / 4 > cap)
-    return fail(g, ORB_E_INVAL, "ORB_MARKERS_TILE_BINS: more than 1638 markers per bin (quarter tile) on average");
+    return fail(g, ORB_E_INVAL, "ORB_MARKERS_TILE_BINS: more than 1638 markers per bin (one radial row of a tile) on average");
   if (n_tiles * cap >= ((int64_t)1 << 32)) return fail(g, ORB_E_INVAL, "tile bins exceed 2^32 records");
   T.cap = (uint32_t)cap;
   T.count = nullptr;

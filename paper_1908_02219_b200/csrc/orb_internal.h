@@ -58,7 +58,7 @@ struct Markers {
 // kTileBinSubs bins of 8 / kTileBinSubs radial rows; bin b = t * kTileBinSubs + sub owns the records
 // [b * cap, b * cap + min(count[b], cap)) of Markers::rec.  count == nullptr: the dense cell-sorted
 // layout of orb_bin.cu (per-cell offsets) is in use instead.
-constexpr int kTileBinSubs = 4;
+constexpr int kTileBinSubs = 8;
 struct TileBins {
   const uint32_t* count;
   uint32_t cap, n_tiles;   // n_tiles: number of BINS (tiles * kTileBinSubs)

@@ -5,13 +5,14 @@
 // layout trades memory for updatability:
 //
 //   slack tile bins   every deposit tile (1 toroidal slab x 8 radial x 16 poloidal cells, the unit
-//                     of work of the tile kernels) is cut into 4 bins of 2 radial rows; bin b owns
-//                     a fixed-capacity segment rec[b * cap .. b * cap + count[b]) of 64-byte marker
-//                     records, in any order.  (Whole-tile bins were measured first: the tile
-//                     kernels take a tile's markers in chunks of 256-384, and a chunk drawn from
-//                     the whole tile spreads its Larmor points over all 288 cells of the halo
-//                     window -- 1.9x slower deposits than chunks of 2-4 radial rows.)
-//                     cap ~ 2 x the mean occupancy + 128.
+//                     of work of the tile kernels) is cut into its 8 radial rows; bin b (1 x 16
+//                     cells) owns a fixed-capacity segment rec[b * cap .. b * cap + count[b]) of
+//                     64-byte marker records, in any order.  The tile kernels take a tile's markers
+//                     in chunks of 256-384, run by run, so a chunk still covers a few whole radial
+//                     rows, as with the dense layout.  (Measured on cfg3: whole-tile bins, whose
+//                     chunks spread their Larmor points over all 288 cells of the halo window, gave
+//                     30.4 ms deposits, quarter-tile bins 18.8 ms, row bins 16.5 ms = the dense
+//                     layout's.)  cap ~ 1.5 x the mean occupancy + 64.
 //   build             ONE pass: slot = atomicAdd(count[tile]); no histogram, no scan.
 //   rebin             after the marker coordinates changed in the records (orb_markers_refresh,
 //                     or a pusher writing them in place): one warp per bin re-derives each

@@ -67,13 +67,17 @@ def _conservation(cfg, m, rho, jpar):
         assert abs(float(jpar.sum().item()) - cfg.q * (m["w"] * m["vpar"]).sum()) <= 1e-11 * scale_j
 
 
+BINNINGS = {"tile_bins": B.ORB_MARKERS_TILE_BINS, "dense": 0}   # bench.py --binning tile | dense
+
+
+@pytest.mark.parametrize("binning", list(BINNINGS))
 @pytest.mark.parametrize("name", ["cfg1", "cfg2", "cfg3"])
-def test_full_grid_against_oracle(name):
+def test_full_grid_against_oracle(name, binning):
     import torch
     cfg = W.CONFIGS[name]
     m = W.generate(cfg)
     d = {f: torch.from_numpy(m[f]).cuda() for f in W.FIELDS}
-    rho, jpar, npts, fallback = _bench_step(cfg, d)
+    rho, jpar, npts, fallback = _bench_step(cfg, d, bind_flags=BINNINGS[binning])
     del d
     rho_o, jpar_o, npts_o, _ = O.deposit_ranges(oracle_geom(cfg), oracle_policy(cfg),
                                                 *(m[f] for f in W.FIELDS), current=cfg.current)
@@ -132,11 +136,12 @@ def _check_grids(rho, jpar, want):
         assert np.abs(gotj - jpar_o).max() <= TOL * np.abs(jpar_o).max(), "jpar plane %d" % k0
 
 
-def test_cfg4_random_order_whole_grid(cfg4_case):
+@pytest.mark.parametrize("binning", list(BINNINGS))
+def test_cfg4_random_order_whole_grid(cfg4_case, binning):
     import torch
     cfg, m, want, npts_o = cfg4_case
     d = {f: torch.from_numpy(m[f]).cuda() for f in W.FIELDS}
-    rho, jpar, npts, fallback = _bench_step(cfg, d)
+    rho, jpar, npts, fallback = _bench_step(cfg, d, bind_flags=BINNINGS[binning])
     del d
     assert npts == npts_o
     assert fallback < 0.01 * npts

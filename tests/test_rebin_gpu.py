@@ -29,14 +29,14 @@ def small(cfg_name, n, **kw):
 
 
 def tile_ids(cfg, s, theta, phi):
-    """Plain definition of the bin (quarter of a deposit tile: 2 radial rows x 16 poloidal cells of
-    one toroidal slab) a marker belongs to (include/orb.h, orb_markers_layout)."""
+    """Plain definition of the bin (one radial row of a deposit tile: 1 x 16 cells of one toroidal
+    slab) a marker belongs to (include/orb.h, orb_markers_layout)."""
     i = np.clip(np.floor(np.clip(s, 0.0, 1.0) * cfg.ns).astype(np.int64), 0, cfg.ns - 1)
     j = np.clip(np.floor(np.mod(theta, W.TWO_PI) * (cfg.ntheta / W.TWO_PI)).astype(np.int64), 0, cfg.ntheta - 1)
     k = np.clip(np.floor(np.mod(phi, W.TWO_PI) * (cfg.nphi / W.TWO_PI)).astype(np.int64), 0, cfg.nphi - 1)
     tiles_i, tiles_j = (cfg.ns + 7) // 8, (cfg.ntheta + 15) // 16
     tile = (k * tiles_i + i // 8) * tiles_j + j // 16
-    return tile * 4 + (i % 8) // 2, tiles_i * tiles_j * cfg.nphi * 4
+    return tile * 8 + i % 8, tiles_i * tiles_j * cfg.nphi * 8
 
 
 def check_bins(cfg, g, m, allow_misplaced=False):
@@ -93,8 +93,9 @@ def test_tile_bins_build_deposit_and_gather(name):
     m = W.generate(cfg)
     d = to_device(m)
     g = bind_tile_bins(cfg, d)
-    # tiny_grid: 5003 markers in 4 tiles of capacity 2048 < mean * 1.25?  (bind refuses then)
-    check_bins(cfg, g, m)
+    # tiny_grid has only 4 of a tile's 8 radial rows: half the bins stay empty, the others exceed
+    # their capacity (1.5 x the mean over ALL bins) and spill into neighbours -- benign
+    check_bins(cfg, g, m, allow_misplaced=(name == "tiny_grid"))
     rho_o, jpar_o, npts_o = run_oracle(cfg, m)
     for algo, flags in TILE_ALGOS.items():
         rho, jpar, npts = deposit(cfg, g, flags)
@@ -194,8 +195,14 @@ def test_rebin_overflows_are_benign():
     rho_o, jpar_o, _ = run_oracle(cfg, m2)
     rho, jpar, _ = deposit(cfg, g)
     assert_parity(rho, rho_o)
-    g.markers_rebin(st)
-    assert g.last_moved() == (misplaced, 0)
+    total = 0
+    for _ in range(4):                       # later rebins finish the move (buffer: n/2 per call)
+        g.markers_rebin(st)
+        moved, left = g.last_moved()
+        total += moved
+        if left == 0:
+            break
+    assert left == 0 and total >= misplaced
     check_bins(cfg, g, m2)
     # crowd: all markers into one cell
     m3 = {f: m2[f].copy() for f in W.FIELDS}
