@@ -40,6 +40,7 @@ constexpr int kCW = kTileJ + 2 * kHaloT;   // cell columns held (24)
 constexpr int kNH = kCH + 3;               // node rows (15)
 constexpr int kNW = kCW + 3;               // node columns (27)
 constexpr unsigned kFull = 0xffffffffu;
+constexpr int kSortCap = 2048;             // markers of a tile that the on-chip cell sort handles
 
 template <int F>
 struct Fields {
@@ -148,6 +149,9 @@ k_gather_tile(const Params P, const Markers M, const uint32_t* __restrict__ cell
   // the swap spreads them over all eight 16-byte bank groups instead of four
   __shared__ __align__(16) double tile[F * kNH * kNW * 4];
   __shared__ uint32_t row_begin[kTileI], row_off[kTileI + 1];
+  __shared__ unsigned int hist[kTileI * kTileJ];
+  __shared__ unsigned int key_rank[kSortCap];
+  __shared__ unsigned short order[kSortCap];
   const int tid = threadIdx.x;
   const int tj = blockIdx.x, ti = blockIdx.y, k = blockIdx.z;
   const int row_base = ti * kTileI - kHaloS;        // radial cell (= first basis index) of cell row 0
@@ -198,10 +202,61 @@ k_gather_tile(const Params P, const Markers M, const uint32_t* __restrict__ cell
   // (uniform over the tile) only tiles that reach the two end cells of the clamped radial basis
   // need the tabulated pieces
   const bool edge = row_base < 2 || row_base + kCH - 1 > P.ns - 3;
-  for (uint32_t v = tid; v < n_tile; v += kThreads) {
+  // Slack-bin layout: the markers of a bin (one radial row of the tile) come in any order.  Lanes of
+  // a warp that work on markers of the same cell read the same nodes (shared-memory broadcast), so
+  // the tile's markers are first put in cell order with a small counting sort on chip (measured on
+  // cfg3: 20.2 ms without it against 13.4 ms from the cell-sorted dense layout).
+  const bool resort = TB.count != nullptr && n_tile <= (uint32_t)kSortCap;
+  if (resort) {
+    for (int x = tid; x < kTileI * kTileJ; x += kThreads) hist[x] = 0;
+    __syncthreads();
+    for (uint32_t v = tid; v < n_tile; v += kThreads) {
+      int r = 0;
+#pragma unroll
+      for (int x = 1; x < kTileI; ++x) r += (v >= row_off[x]) ? 1 : 0;
+      const int64_t p = (int64_t)row_begin[r] + (v - row_off[r]);
+      const double2 st = __ldg(reinterpret_cast<const double2*>(M.rec + p * kRecDoubles));
+      int ci = (int)(fmin(fmax(st.x, 0.0), 1.0) * (double)P.ns) - ti * kTileI;
+      int cj = (int)(wrap_2pi(st.y) * P.nth_scale) - tj * kTileJ;
+      ci = min(max(ci, 0), kTileI - 1);      // (a mis-binned marker just lands in an edge cell)
+      cj = min(max(cj, 0), kTileJ - 1);
+      const int c = ci * kTileJ + cj;
+      const unsigned int rank = atomicAdd(&hist[c], 1u);
+      key_rank[v] = (unsigned short)c | (rank << 16);
+    }
+    __syncthreads();
+    if (tid < 32) {   // exclusive scan of the 128 cell counts
+      unsigned int c4[4], sum = 0;
+#pragma unroll
+      for (int x = 0; x < 4; ++x) {
+        c4[x] = hist[tid * 4 + x];
+        sum += c4[x];
+      }
+      unsigned int inc = sum;
+#pragma unroll
+      for (int o = 1; o < 32; o <<= 1) {
+        const unsigned int t = __shfl_up_sync(kFull, inc, o);
+        if (tid >= o) inc += t;
+      }
+      unsigned int ex = inc - sum;
+#pragma unroll
+      for (int x = 0; x < 4; ++x) {
+        hist[tid * 4 + x] = ex;
+        ex += c4[x];
+      }
+    }
+    __syncthreads();
+    for (uint32_t v = tid; v < n_tile; v += kThreads) {
+      const unsigned int kr = key_rank[v];
+      order[hist[kr & 0xffffu] + (kr >> 16)] = (unsigned short)v;
+    }
+    __syncthreads();
+  }
+  for (uint32_t x = tid; x < n_tile; x += kThreads) {
+    const uint32_t v = resort ? (uint32_t)order[x] : x;
     int r = 0;
 #pragma unroll
-    for (int x = 1; x < kTileI; ++x) r += (v >= row_off[x]) ? 1 : 0;
+    for (int y = 1; y < kTileI; ++y) r += (v >= row_off[y]) ? 1 : 0;
     const int64_t p = (int64_t)row_begin[r] + (v - row_off[r]);
     const MarkerData m = load_marker(M, p);
     const GuidingCentre g = guiding_centre(P, m.s, m.th, m.mu);
