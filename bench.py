@@ -363,6 +363,68 @@ def run_ours(args):
         del fields
         torch.cuda.empty_cache()
 
+    # ---- NEXT-2 leg: incremental re-binning of the slack bins after a synthetic push, and
+    # NEXT-3 leg: the materialised-ring-data / cell-owner path on the same markers (single species)
+    rebin = ring = None
+    if not args.no_next_legs and NS == 1:
+        sp = species[0]
+        ev = lambda: torch.cuda.Event(enable_timing=True)  # noqa: E731
+        if args.binning == "tile" and sp.bind_flags == B.ORB_MARKERS_TILE_BINS:
+            rebin = {"what": "orb_markers_rebin after a seeded fraction of the markers jumped 24 "
+                             "theta* cells (1.5 tiles); refresh = orb_markers_refresh (records <- bound arrays)",
+                     "build_ms": bin_ms, "cases": []}
+            gen = torch.Generator(device=dev)
+            gen.manual_seed(99 + rank)
+            theta0 = sp.d["theta"].clone()
+            for frac in (0.0, 0.01, 0.1, 0.5):
+                sel = torch.rand(sp.cfg.n_markers, device=dev, generator=gen) < frac
+                sp.d["theta"][sel] += 24.0 * (W.TWO_PI / sp.cfg.ntheta)
+                e0, e1, e2 = ev(), ev(), ev()
+                e0.record(stream)
+                sp.g.markers_refresh(st)
+                e1.record(stream)
+                sp.g.markers_rebin(st)
+                e2.record(stream)
+                torch.cuda.synchronize()
+                moved, left = sp.g.last_moved()
+                rebin["cases"].append({"moved_fraction": frac, "moved": moved, "left_in_place": left,
+                                       "refresh_ms": e0.elapsed_time(e1), "rebin_ms": e1.elapsed_time(e2)})
+            e0, e1 = ev(), ev()
+            sp.g.grid_zero(rho, jpar, st)
+            e0.record(stream)
+            sp.g.deposit(rho, jpar if sp.cfg.current else None, sp.pol, st)
+            e1.record(stream)
+            torch.cuda.synchronize()
+            rebin["deposit_after_rebin_ms"] = e0.elapsed_time(e1)
+            w_now = float(rho.sum().item())
+            rebin["charge_conservation_rel"] = abs(w_now - w_sum) / w_abs
+            sp.d["theta"].copy_(theta0)
+            del theta0
+            sp.bind()
+            sp.g.markers_bin(st)
+        try:
+            nl_cap = sp.cfg.n_max if sp.cfg.adaptive else sp.cfg.n_fixed
+            sp.g.ring_reserve(sp.cfg.n_markers, min(npts_step + 1024, sp.cfg.n_markers * nl_cap))
+            pol_ring = B.policy_for(sp.cfg, flags=B.ORB_DEPOSIT_ALGO_RING_DATA)
+            ts = []
+            for _ in range(3):
+                sp.g.grid_zero(rho, jpar, st)
+                e0, e1 = ev(), ev()
+                e0.record(stream)
+                sp.g.deposit(rho, jpar if sp.cfg.current else None, pol_ring, st)
+                e1.record(stream)
+                torch.cuda.synchronize()
+                ts.append(e0.elapsed_time(e1))
+            ring = {"what": "ORB_DEPOSIT_ALGO_RING_DATA: build Larmor ring data in HBM, bucket-sort the "
+                            "points by cell, cell-owner loop (PAPER.md:73-75); no marker binning needed",
+                    "ms": min(ts), "value": npts_step / (min(ts) * 1e-3), "unit": UNIT,
+                    "charge_conservation_rel": abs(float(rho.sum().item()) - w_sum) / w_abs,
+                    "compare_with_step_ms": job_ms / K}
+            sp.g.ring_reserve(0, 0)
+        except B.OrbError as e:  # noqa: PERF203
+            ring = {"unavailable": str(e)}
+        torch.cuda.empty_cache()
+
     # ---- e2e: HOST marker arrays -> orb_deposit_host -> HOST grids, every step
     E = max(1, min(args.e2e_steps, K))
     rho_h = [torch.empty(shape, dtype=torch.float64, pin_memory=True) for _ in species]
@@ -457,6 +519,10 @@ def run_ours(args):
             "checks": {"charge_conservation_rel": conservation,
                        "e2e_charge_conservation_rel": e2e_conservation},
         }
+        if rebin:
+            line["rebin"] = rebin
+        if ring:
+            line["ring_data"] = ring
         if gather:
             g_ach = gather["algorithmic_bytes"] / (gather["ms"] * 1e-3) / 1e9
             line["gather"] = {
@@ -499,6 +565,8 @@ def main(argv=None):
     ap.add_argument("--binning", default="tile", choices=["tile", "dense"],
                     help="marker binning of the step: slack tile bins built in one pass "
                          "(ORB_MARKERS_TILE_BINS) or the dense counting sort by cell")
+    ap.add_argument("--no-next-legs", action="store_true",
+                    help="skip the incremental re-binning (NEXT-2) and ring-data (NEXT-3) legs")
     ap.add_argument("--no-gather", action="store_true", help="skip the orb_gather (NEXT-1) leg")
     args = ap.parse_args(argv)
     if args.warmup < 3 and args.impl == "ours":

@@ -159,7 +159,8 @@ int orb_reserve(orb_grid_t *g, int64_t n);
 
 /* Reserves the scratch of ORB_DEPOSIT_ALGO_RING_DATA: Larmor ring data for up to n_points Larmor
  * points (2 x 48 bytes each: in marker order and sorted by cell) of up to n_markers markers.
- * Allocates (synchronises); call it outside timed / captured regions.  Points beyond n_points are
+ * Allocates (synchronises); call it outside timed / captured regions; (0, 0) frees the scratch.
+ * Points beyond n_points are
  * still deposited (directly, with global atomics) and counted by orb_last_fallback_points. */
 int orb_ring_reserve(orb_grid_t *g, int64_t n_markers, int64_t n_points);
 

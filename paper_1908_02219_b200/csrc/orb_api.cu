@@ -442,6 +442,10 @@ int orb_ring_reserve(orb_grid_t* g, int64_t n_markers, int64_t n_points) {
     return fail(g, ORB_E_INVAL, "orb_ring_reserve: counts out of range");
   DeviceGuard dg(g->desc.device);
   if (!dg.ok) return fail(g, ORB_E_CUDA, "cudaSetDevice");
+  if (n_markers == 0 && n_points == 0) {   // release the scratch
+    free_ringdata(g);
+    return ORB_OK;
+  }
   if (n_markers <= g->ringdata.markers && n_points <= g->ringdata.capacity) return ORB_OK;
   free_ringdata(g);
   RingScratch R;
