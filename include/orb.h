@@ -88,12 +88,14 @@ enum { ORB_NL_FIXED = 0, ORB_NL_ADAPTIVE = 1 };
                                         shared-memory tile kernel                              */
 #define ORB_DEPOSIT_ALGO_TILE_V4 0x8u /* force the one-block-per-tile kernel (all warps run all
                                         phases; several blocks per SM)                          */
-#define ORB_DEPOSIT_ALGO_TILE_WS 0x10u /* force the persistent warp-specialised tile kernel
-                                        (producer / consumer warps, one block per SM)
-                                        By default the library picks between the two tile
-                                        kernels by N_L policy: persistent for fixed N_L <= 4,
-                                        one-block-per-tile for larger or adaptive N_L.            */
-
+#define ORB_DEPOSIT_ALGO_TILE_WS 0x10u /* force the first persistent warp-specialised kernel (64-byte
+                                        operand records, chunks of 256 markers); kept for
+                                        comparison.  By default the library picks by N_L policy:
+                                        the persistent kernel with 16-byte point records and
+                                        whole-tile-sized chunks (orb_deposit_ws2.cu) for fixed
+                                        N_L <= 4, the one-block-per-tile kernel for larger or
+                                        adaptive N_L.                                             */
+#define ORB_DEPOSIT_ALGO_TILE_WS2 0x40u /* (no effect: names the default for fixed N_L <= 4)       */
 #define ORB_DEPOSIT_ALGO_RING_DATA 0x20u /* the paper's own organisation, as a
                                         measured alternative: materialise the Larmor ring data in
                                         device memory, bucket-sort the Larmor POINTS by field

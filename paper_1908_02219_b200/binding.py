@@ -19,6 +19,7 @@ ORB_DEPOSIT_ALGO_ATOMIC = 0x4
 ORB_DEPOSIT_ALGO_TILE_V4 = 0x8
 ORB_DEPOSIT_ALGO_TILE_WS = 0x10
 ORB_DEPOSIT_ALGO_RING_DATA = 0x20
+ORB_DEPOSIT_ALGO_TILE_WS2 = 0x40
 ORB_MARKERS_SORTED = 0x1
 ORB_MARKERS_TILE_BINS = 0x2
 ORB_MAX_NL = 32

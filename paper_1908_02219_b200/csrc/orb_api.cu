@@ -524,11 +524,15 @@ int orb_deposit(orb_grid_t* g, double* rho, double* jpar, const orb_nl_policy_t*
     l = launch_deposit_atomic(P, M, rho, jpar, g->d_points, st);
   } else if (tile_v4 || (!tile_v5 && (P.adaptive || P.n_fixed > 4))) {
     // N_L > 4 or adaptive: the one-block-per-tile kernel, whose point slots are filled by a
-    // prefix sum over the markers, keeps its lanes busier than the persistent kernel's
+    // prefix sum over the markers, keeps its lanes busier than the persistent kernels'
     // unit hand-over (measured: cfg2 5.5 vs 7.5 ms, cfg4 70 vs 111 ms)
     l = launch_deposit_tile(P, M, g->bin.cell_start, TB, rho, jpar, g->d_points, st);
-  } else {
+  } else if (tile_v5) {
     l = launch_deposit_ws(P, M, g->bin.cell_start, TB, rho, jpar, g->d_points, g->sms, st);
+  } else {
+    // fixed N_L <= 4: the persistent kernel with whole-tile-sized chunks (cfg3 15.1 vs 16.4 ms,
+    // cfg1 2.9 vs 3.6 ms against ORB_DEPOSIT_ALGO_TILE_WS)
+    l = launch_deposit_ws2(P, M, g->bin.cell_start, TB, rho, jpar, g->d_points, g->sms, st);
   }
   if (l < 0) return fail(g, ORB_E_CUDA, "deposit launch", cudaGetLastError());
   g->launches += l;

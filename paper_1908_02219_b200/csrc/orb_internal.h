@@ -116,6 +116,11 @@ struct RingScratch {
 int launch_deposit_ringdata(const Params& P, const Markers& M, const RingScratch& R, double* rho,
                             double* jpar, unsigned long long* d_points, cudaStream_t st);
 
+// v6: v5's pipeline with whole-tile chunks and 16-byte point records (orb_deposit_ws2.cu); fixed N_L <= 4
+int launch_deposit_ws2(const Params& P, const Markers& M, const uint32_t* cell_start,
+                       const TileBins& TB, double* rho, double* jpar, unsigned long long* d_points,
+                       int sms, cudaStream_t st);
+
 // ring table (cos, sin)(alpha0 + 2 pi l / N), built on the device (orb_ring.cu)
 int launch_ring_table(double2* ring, double alpha0, cudaStream_t st);
 

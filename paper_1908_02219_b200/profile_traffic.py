@@ -19,7 +19,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 ROOT = os.path.dirname(HERE)
 OUT = os.path.join(ROOT, "profiles", "r02_traffic.json")
-KERNEL_SOURCES = ("orb_deposit_ws.cu", "orb_deposit_tile.cu", "orb_geom.cuh")
+KERNEL_SOURCES = ("orb_deposit_ws2.cu", "orb_deposit_ws.cu", "orb_deposit_tile.cu", "orb_geom.cuh")
 UNIT = {"byte": 1.0, "Kbyte": 1e3, "Mbyte": 1e6, "Gbyte": 1e9, "Tbyte": 1e12}
 
 

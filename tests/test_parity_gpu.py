@@ -18,9 +18,10 @@ ALGOS = {
     "atomic": B.ORB_DEPOSIT_ALGO_ATOMIC,
     "atomic_nobin": B.ORB_DEPOSIT_ALGO_ATOMIC | B.ORB_DEPOSIT_NO_BIN,
     "tile_v4": B.ORB_DEPOSIT_ALGO_TILE_V4,       # one block per tile
-    "tile_ws": B.ORB_DEPOSIT_ALGO_TILE_WS,       # persistent, warp-specialised
+    "tile_ws": B.ORB_DEPOSIT_ALGO_TILE_WS,       # persistent, warp-specialised, 64-byte operand records
     "ring_data": B.ORB_DEPOSIT_ALGO_RING_DATA,   # NEXT-3: Larmor ring data + cell-owner loop
-    "tile": 0,          # the product path: the library picks between the two by N_L policy
+    "tile": 0,          # the product path: the library picks by N_L policy (fixed N_L <= 4: the
+                        # persistent kernel with whole-tile chunks, orb_deposit_ws2.cu)
 }
 
 
