@@ -237,7 +237,9 @@ class Species:
 
 def deposit_kernel_name(cfg):
     """The tile kernel orb_deposit picks for this N_L policy (csrc/orb_api.cu)."""
-    return "k_deposit_tile" if (cfg.adaptive or cfg.n_fixed > 4) else "k_deposit_ws2"
+    if cfg.adaptive or cfg.n_fixed > 4:
+        return "k_deposit_tile"
+    return "k_deposit_ws<" if cfg.n_fixed == 1 else "k_deposit_ws2"
 
 
 def run_ours(args):

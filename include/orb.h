@@ -93,9 +93,9 @@ enum { ORB_NL_FIXED = 0, ORB_NL_ADAPTIVE = 1 };
                                         comparison.  By default the library picks by N_L policy:
                                         the persistent kernel with 16-byte point records and
                                         whole-tile-sized chunks (orb_deposit_ws2.cu) for fixed
-                                        N_L <= 4, the one-block-per-tile kernel for larger or
-                                        adaptive N_L.                                             */
-#define ORB_DEPOSIT_ALGO_TILE_WS2 0x40u /* (no effect: names the default for fixed N_L <= 4)       */
+                                        N_L = 2..4, this one for N_L = 1, the one-block-per-tile
+                                        kernel for larger or adaptive N_L.                        */
+#define ORB_DEPOSIT_ALGO_TILE_WS2 0x40u /* (no effect: names the default for fixed N_L = 2..4)     */
 #define ORB_DEPOSIT_ALGO_RING_DATA 0x20u /* the paper's own organisation, as a
                                         measured alternative: materialise the Larmor ring data in
                                         device memory, bucket-sort the Larmor POINTS by field

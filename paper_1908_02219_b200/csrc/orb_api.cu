@@ -527,10 +527,12 @@ int orb_deposit(orb_grid_t* g, double* rho, double* jpar, const orb_nl_policy_t*
     // prefix sum over the markers, keeps its lanes busier than the persistent kernels'
     // unit hand-over (measured: cfg2 5.5 vs 7.5 ms, cfg4 70 vs 111 ms)
     l = launch_deposit_tile(P, M, g->bin.cell_start, TB, rho, jpar, g->d_points, st);
-  } else if (tile_v5) {
+  } else if (tile_v5 || P.n_fixed == 1) {
+    // N_L = 1 (drift-kinetic species): one point per marker slot; the 256-marker chunks of the first
+    // persistent kernel are faster there (single_node electrons: 2.65 vs 3.19 ms)
     l = launch_deposit_ws(P, M, g->bin.cell_start, TB, rho, jpar, g->d_points, g->sms, st);
   } else {
-    // fixed N_L <= 4: the persistent kernel with whole-tile-sized chunks (cfg3 15.1 vs 16.4 ms,
+    // fixed N_L = 2..4: the persistent kernel with whole-tile-sized chunks (cfg3 15.1 vs 16.4 ms,
     // cfg1 2.9 vs 3.6 ms against ORB_DEPOSIT_ALGO_TILE_WS)
     l = launch_deposit_ws2(P, M, g->bin.cell_start, TB, rho, jpar, g->d_points, g->sms, st);
   }

@@ -192,7 +192,7 @@ def test_sorted_flag_on_unsorted_markers_stays_correct(oracle_results):
     result must still be the oracle's (sorted == unsorted)."""
     for name in ("cfg3_small", "cfg4_small"):
         cfg, m, (rho_o, jpar_o, npts_o) = get_case(name, oracle_results)
-        for algo in ("tile_ws", "tile_v4"):
+        for algo in ("tile", "tile_ws", "tile_v4"):
             rho, jpar, npts = run_gpu(cfg, m, flags=ALGOS[algo], bind_flags=B.ORB_MARKERS_SORTED)
             assert npts == npts_o
             assert_parity(rho, rho_o, "%s/%s rho" % (name, algo))

@@ -21,7 +21,8 @@ from test_gather_gpu import fields_for, gather_oracle
 
 pytestmark = pytest.mark.gpu
 
-TILE_ALGOS = {"tile_v4": B.ORB_DEPOSIT_ALGO_TILE_V4, "tile_ws": B.ORB_DEPOSIT_ALGO_TILE_WS, "tile": 0}
+TILE_ALGOS = {"tile_v4": B.ORB_DEPOSIT_ALGO_TILE_V4, "tile_ws": B.ORB_DEPOSIT_ALGO_TILE_WS,
+              "tile": 0}     # "tile": the library's pick (fixed N_L <= 4: k_deposit_ws2)
 
 
 def small(cfg_name, n, **kw):
