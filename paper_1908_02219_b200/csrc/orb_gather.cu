@@ -40,7 +40,9 @@ constexpr int kCW = kTileJ + 2 * kHaloT;   // cell columns held (24)
 constexpr int kNH = kCH + 3;               // node rows (15)
 constexpr int kNW = kCW + 3;               // node columns (27)
 constexpr unsigned kFull = 0xffffffffu;
-constexpr int kSortCap = 2048;             // markers of a tile that the on-chip cell sort handles
+constexpr int kSortCap = 2048;             // markers of a tile that the on-chip sort handles
+constexpr int kSortClasses = 8;            // N_L classes of the sort key: N_L <= 4, <= 8, ..., > 28
+constexpr int kSortBins = kSortClasses * kTileI * kTileJ;   // (N_L class, cell) bins: 1024
 
 template <int F>
 struct Fields {
@@ -149,7 +151,8 @@ k_gather_tile(const Params P, const Markers M, const uint32_t* __restrict__ cell
   // the swap spreads them over all eight 16-byte bank groups instead of four
   __shared__ __align__(16) double tile[F * kNH * kNW * 4];
   __shared__ uint32_t row_begin[kTileI], row_off[kTileI + 1];
-  __shared__ unsigned int hist[kTileI * kTileJ];
+  __shared__ unsigned int hist[kSortBins];
+  __shared__ unsigned int warp_tot[kThreads / 32];
   __shared__ unsigned int key_rank[kSortCap];
   __shared__ unsigned short order[kSortCap];
   const int tid = threadIdx.x;
@@ -202,30 +205,35 @@ k_gather_tile(const Params P, const Markers M, const uint32_t* __restrict__ cell
   // (uniform over the tile) only tiles that reach the two end cells of the clamped radial basis
   // need the tabulated pieces
   const bool edge = row_base < 2 || row_base + kCH - 1 > P.ns - 3;
-  // Slack-bin layout: the markers of a bin (one radial row of the tile) come in any order.  Lanes of
-  // a warp that work on markers of the same cell read the same nodes (shared-memory broadcast), so
-  // the tile's markers are first put in cell order with a small counting sort on chip (measured on
-  // cfg3: 20.2 ms without it against 13.4 ms from the cell-sorted dense layout).
-  const bool resort = TB.count != nullptr && n_tile <= (uint32_t)kSortCap;
+  // Order of work inside the tile.  Lanes of a warp that work on markers of the same cell read the
+  // same nodes (shared-memory broadcast), and lanes whose markers have the same N_L leave the ring
+  // loop together.  The dense cell-sorted layout gives the first for free; for slack bins (markers
+  // of a tile row in any order) and for adaptive N_L the tile's markers are first put in
+  // (N_L class, cell) order with a small counting sort on chip.  Measured: cfg3 from slack bins
+  // 20.2 -> 14.5 ms (13.4 ms from the dense layout); cfg4 (N_L = 4..16) 112 -> see DESIGN.md 6.4.
+  const bool resort = (TB.count != nullptr || P.adaptive) && n_tile <= (uint32_t)kSortCap;
   if (resort) {
-    for (int x = tid; x < kTileI * kTileJ; x += kThreads) hist[x] = 0;
+    for (int x = tid; x < kSortBins; x += kThreads) hist[x] = 0;
     __syncthreads();
     for (uint32_t v = tid; v < n_tile; v += kThreads) {
       int r = 0;
 #pragma unroll
       for (int x = 1; x < kTileI; ++x) r += (v >= row_off[x]) ? 1 : 0;
       const int64_t p = (int64_t)row_begin[r] + (v - row_off[r]);
-      const double2 st = __ldg(reinterpret_cast<const double2*>(M.rec + p * kRecDoubles));
-      int ci = (int)(fmin(fmax(st.x, 0.0), 1.0) * (double)P.ns) - ti * kTileI;
-      int cj = (int)(wrap_2pi(st.y) * P.nth_scale) - tj * kTileJ;
+      const MarkerData m = load_marker(M, p);
+      int ci = (int)(fmin(fmax(m.s, 0.0), 1.0) * (double)P.ns) - ti * kTileI;
+      int cj = (int)(wrap_2pi(m.th) * P.nth_scale) - tj * kTileJ;
       ci = min(max(ci, 0), kTileI - 1);      // (a mis-binned marker just lands in an edge cell)
       cj = min(max(cj, 0), kTileJ - 1);
-      const int c = ci * kTileJ + cj;
+      int cls = 0;
+      if (P.adaptive) cls = min((guiding_centre(P, m.s, m.th, m.mu).n - 1) >> 2, kSortClasses - 1);
+      const int c = (cls * kTileI + ci) * kTileJ + cj;
       const unsigned int rank = atomicAdd(&hist[c], 1u);
-      key_rank[v] = (unsigned short)c | (rank << 16);
+      key_rank[v] = (unsigned int)c | (rank << 16);
     }
     __syncthreads();
-    if (tid < 32) {   // exclusive scan of the 128 cell counts
+    {   // exclusive scan of the kSortBins counts: 4 per thread, warp scan, warp totals
+      static_assert(kSortBins == 4 * kThreads, "one thread scans 4 bins");
       unsigned int c4[4], sum = 0;
 #pragma unroll
       for (int x = 0; x < 4; ++x) {
@@ -236,9 +244,13 @@ k_gather_tile(const Params P, const Markers M, const uint32_t* __restrict__ cell
 #pragma unroll
       for (int o = 1; o < 32; o <<= 1) {
         const unsigned int t = __shfl_up_sync(kFull, inc, o);
-        if (tid >= o) inc += t;
+        if ((tid & 31) >= o) inc += t;
       }
-      unsigned int ex = inc - sum;
+      if ((tid & 31) == 31) warp_tot[tid >> 5] = inc;
+      __syncthreads();
+      unsigned int base = 0;
+      for (int w = 0; w < (tid >> 5); ++w) base += warp_tot[w];
+      unsigned int ex = base + inc - sum;
 #pragma unroll
       for (int x = 0; x < 4; ++x) {
         hist[tid * 4 + x] = ex;
