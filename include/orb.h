@@ -262,9 +262,13 @@ int orb_last_fallback_points(orb_grid_t *g, int64_t *n_points);
  * NULL) to library-owned device buffers, binds, deposits into zeroed device grids
  * and copies rho (and jpar) back into the host arrays, which are OVERWRITTEN.
  * Above 2^22 markers the work is pipelined on two library-owned streams: the markers travel in
- * 8 slices and the copy of slice i+1 overlaps binning and deposition of slice i (the call is
- * bound by the host link: 48 B per marker); use pinned host memory for the overlap to happen.
- * Synchronous.  Leaves the handle bound to the library's own device copies.
+ * 8 slices; each slice is appended to the slack tile bins (ORB_MARKERS_TILE_BINS layout, sized for
+ * all n markers) as soon as its copy has landed, and the deposit kernel runs once per GROUP of
+ * slices (6 + 2), so that a tile is visited twice per call, not once per slice; the first group's
+ * deposit overlaps the last two copies (the call is bound by the host link: 48 B per marker).
+ * With ORB_DEPOSIT_NO_BIN, _ALGO_ATOMIC or _ALGO_RING_DATA every slice is deposited on its own.
+ * Use pinned host memory for the overlap to happen.
+ * Synchronous.  Leaves the handle bound to the library's own device copies (not binned).
  * h2d_bytes / d2h_bytes (optional) receive the bytes moved. */
 int orb_deposit_host(orb_grid_t *g, int64_t n, const double *s, const double *theta,
                      const double *phi, const double *vpar, const double *mu, const double *w,

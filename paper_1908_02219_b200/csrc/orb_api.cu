@@ -14,6 +14,12 @@ using namespace orb;
 // orb_deposit_host pipelines the markers in this many slices: the host->device copy of slice
 // i+1 overlaps binning and deposition of slice i (the call is PCIe-bound: 48 B per marker)
 constexpr int kHostSlices = 8;
+// ... and deposits them in this many groups of slices: group k ends after slice kHostGroupEnd[k].
+// A deposit over all tiles costs ~5.5 ms + 9.6 ms x (fraction of the markers) on cfg3, so few groups;
+// measured e2e ms per call on cfg3: {6, 8} 71.5, {7, 8} 78.1, one deposit per slice 73.5,
+// 16 slices {12, 16} 71.5, {13, 16} 74.6 (profiles/r02_experiments.md section 7).
+constexpr int kHostGroups = 2;
+constexpr int kHostGroupEnd[kHostGroups] = {6, kHostSlices};
 
 struct orb_grid {
   orb_grid_desc_t desc;
@@ -778,6 +784,22 @@ int orb_deposit_host(orb_grid_t* g, int64_t n, const double* s, const double* th
     if (rc != ORB_OK) return rc;
     ORB_CUDA(g, cudaMemsetAsync(g->d_points, 0, kCounters * sizeof(unsigned long long), st));
   }
+  // The whole device copy is bound once with slack tile bins sized for all n markers.  Each slice
+  // is APPENDED to the bins as soon as its copy has landed (the one-pass build claims bin slots
+  // with atomics, so it does not care in how many launches the markers come); the deposit kernel
+  // runs once per GROUP of slices, so a tile is zeroed, walked and flushed kHostGroups times per
+  // call, not once per slice.  The first group's deposit overlaps the copies of the last slices.
+  // (The algorithms that read the bound arrays themselves — ORB_DEPOSIT_NO_BIN, _ALGO_ATOMIC,
+  // _ALGO_RING_DATA — have no per-tile cost and are run slice by slice.)
+  const bool by_slice =
+      (pol->flags & (ORB_DEPOSIT_NO_BIN | ORB_DEPOSIT_ALGO_ATOMIC | ORB_DEPOSIT_ALGO_RING_DATA)) != 0;
+  if (n > 0 && !by_slice) {
+    rc = orb_markers_bind(g, n, g->hbuf[0], g->hbuf[1], g->hbuf[2], vpar ? g->hbuf[3] : nullptr,
+                          g->hbuf[4], g->hbuf[5], ORB_MARKERS_TILE_BINS);
+    if (rc != ORB_OK) return rc;
+  }
+  const Params Pb = make_params(g, nullptr);
+  bool first_of_group = true, first_group = true;
   for (int i = 0; i < n_slices && n > 0; ++i) {
     const int64_t off = i * per;
     const int64_t len = (off + per <= n ? per : n - off);
@@ -790,15 +812,45 @@ int orb_deposit_host(orb_grid_t* g, int64_t n, const double* s, const double* th
     }
     ORB_CUDA(g, cudaEventRecord(g->hevent[i], s_copy));
     ORB_CUDA(g, cudaStreamWaitEvent(st, g->hevent[i], 0));
-    rc = orb_markers_bind(g, len, g->hbuf[0] + off, g->hbuf[1] + off, g->hbuf[2] + off,
-                          vpar ? g->hbuf[3] + off : nullptr, g->hbuf[4] + off, g->hbuf[5] + off, 0);
-    if (rc != ORB_OK) return rc;
+    if (by_slice) {
+      rc = orb_markers_bind(g, len, g->hbuf[0] + off, g->hbuf[1] + off, g->hbuf[2] + off,
+                            vpar ? g->hbuf[3] + off : nullptr, g->hbuf[4] + off, g->hbuf[5] + off, 0);
+      if (rc != ORB_OK) return rc;
+      orb_nl_policy_t p2 = *pol;
+      if (i == 0) p2.flags |= ORB_DEPOSIT_ZERO_FIRST; else p2.flags &= ~ORB_DEPOSIT_ZERO_FIRST;
+      g->keep_counters = i > 0;
+      rc = orb_deposit(g, rho_d, jpar_d, &p2, st);
+      g->keep_counters = false;
+      if (rc != ORB_OK) return rc;
+      continue;
+    }
+    Markers M = g->bound;
+    M.s += off;
+    M.th += off;
+    M.ph += off;
+    if (M.vpar) M.vpar += off;
+    M.mu += off;
+    M.w += off;
+    M.rec = nullptr;
+    M.n = len;
+    int l = launch_tilebin_build(Pb, M, g->tb, g->tb_count, g->tb_rec, st, off, !first_of_group);
+    if (l < 0) return fail(g, ORB_E_CUDA, "tile-bin build launch", cudaGetLastError());
+    g->launches += l;
+    first_of_group = false;
+    const bool last = off + len >= n;
+    bool group_end = last;
+    for (int k = 0; k < kHostGroups; ++k) group_end = group_end || (i + 1 == kHostGroupEnd[k]);
+    if (!group_end) continue;
     orb_nl_policy_t p2 = *pol;
-    if (i == 0) p2.flags |= ORB_DEPOSIT_ZERO_FIRST; else p2.flags &= ~ORB_DEPOSIT_ZERO_FIRST;
-    g->keep_counters = i > 0;
+    if (first_group) p2.flags |= ORB_DEPOSIT_ZERO_FIRST; else p2.flags &= ~ORB_DEPOSIT_ZERO_FIRST;
+    g->keep_counters = !first_group;
+    g->binned = true;          // the bins hold exactly this group's markers
     rc = orb_deposit(g, rho_d, jpar_d, &p2, st);
     g->keep_counters = false;
+    g->binned = false;
     if (rc != ORB_OK) return rc;
+    first_group = false;
+    first_of_group = true;
   }
   ORB_CUDA(g, cudaMemcpyAsync(rho_host, rho_d, (size_t)g->nnodes * sizeof(double),
                               cudaMemcpyDeviceToHost, st));
@@ -809,10 +861,12 @@ int orb_deposit_host(orb_grid_t* g, int64_t n, const double* s, const double* th
     down += g->nnodes * (int64_t)sizeof(double);
   }
   ORB_CUDA(g, cudaStreamSynchronize(st));
-  // leave the handle bound to the whole device copy (not binned)
-  rc = orb_markers_bind(g, n, g->hbuf[0], g->hbuf[1], g->hbuf[2], vpar ? g->hbuf[3] : nullptr,
-                        g->hbuf[4], g->hbuf[5], 0);
-  if (rc != ORB_OK) return rc;
+  // the handle stays bound to the whole device copy, not binned (the bins hold the last group)
+  if (n == 0 || by_slice) {
+    rc = orb_markers_bind(g, n, g->hbuf[0], g->hbuf[1], g->hbuf[2], vpar ? g->hbuf[3] : nullptr,
+                          g->hbuf[4], g->hbuf[5], 0);
+    if (rc != ORB_OK) return rc;
+  }
   if (n_points) {
     unsigned long long v = 0;
     ORB_CUDA(g, cudaMemcpy(&v, g->d_points, sizeof(v), cudaMemcpyDeviceToHost));

@@ -95,8 +95,10 @@ int launch_gather(const Params& P, const Markers& M, const uint32_t* cell_start,
                   bool tiled, cudaStream_t st);
 
 // slack tile bins: one-pass build, refresh of the records from the bound arrays, incremental rebin
+// base = index of M's first marker in the bound arrays (kept in each record); append = add to the
+// bins as they stand instead of emptying them first (orb_deposit_host bins slice by slice)
 int launch_tilebin_build(const Params& P, const Markers& M, const TileBins& T, uint32_t* count, double* rec,
-                         cudaStream_t st);
+                         cudaStream_t st, int64_t base = 0, bool append = false);
 int launch_tilebin_refresh(const Markers& M, const TileBins& T, const uint32_t* count, double* rec,
                            cudaStream_t st);
 int launch_tilebin_rebin(const Params& P, const TileBins& T, uint32_t* count, double* rec, double* movers,

@@ -71,7 +71,7 @@ __device__ __forceinline__ void store_record(double* __restrict__ out, double s,
 // (2.3 TB/s with one marker per thread), so more independent chains per thread is what helps.
 __global__ void __launch_bounds__(256)
 k_tilebin_build(const Params P, const Markers M, const TileBins T, uint32_t* __restrict__ count,
-                double* __restrict__ rec) {
+                double* __restrict__ rec, const int64_t base) {
   const int64_t p = 2 * ((int64_t)blockIdx.x * blockDim.x + threadIdx.x);
   if (p >= M.n) return;
   if (p + 1 < M.n) {
@@ -86,10 +86,10 @@ k_tilebin_build(const Params P, const Markers M, const TileBins T, uint32_t* __r
     const int64_t d0 = claim_slot(count, t0, T.n_tiles, T.cap);
     const int64_t d1 = claim_slot(count, t1, T.n_tiles, T.cap);
     if (d0 >= 0)
-      store_record(rec + d0 * kRecDoubles, s.x, th.x, ph.x, vp.x, mu.x, w.x, __longlong_as_double((long long)p));
+      store_record(rec + d0 * kRecDoubles, s.x, th.x, ph.x, vp.x, mu.x, w.x, __longlong_as_double((long long)(base + p)));
     if (d1 >= 0)
       store_record(rec + d1 * kRecDoubles, s.y, th.y, ph.y, vp.y, mu.y, w.y,
-                   __longlong_as_double((long long)(p + 1)));
+                   __longlong_as_double((long long)(base + p + 1)));
     return;
   }
   const double s = __ldg(M.s + p), th = __ldg(M.th + p), ph = __ldg(M.ph + p);
@@ -97,7 +97,7 @@ k_tilebin_build(const Params P, const Markers M, const TileBins T, uint32_t* __r
   const int64_t dst = claim_slot(count, t, T.n_tiles, T.cap);
   if (dst < 0) return;
   store_record(rec + dst * kRecDoubles, s, th, ph, M.vpar ? __ldg(M.vpar + p) : 0.0, __ldg(M.mu + p),
-               __ldg(M.w + p), __longlong_as_double((long long)p));
+               __ldg(M.w + p), __longlong_as_double((long long)(base + p)));
 }
 
 // records <- current values of the bound arrays (by the original index kept in the record)
@@ -250,11 +250,13 @@ k_tilebin_insert(const TileBins T, uint32_t* __restrict__ count, double* __restr
 }  // namespace
 
 int launch_tilebin_build(const Params& P, const Markers& M, const TileBins& T, uint32_t* count, double* rec,
-                         cudaStream_t st) {
-  if (cudaMemsetAsync(count, 0, (size_t)T.n_tiles * sizeof(uint32_t), st) != cudaSuccess) return -1;
+                         cudaStream_t st, int64_t base, bool append) {
+  if (!append &&
+      cudaMemsetAsync(count, 0, (size_t)T.n_tiles * sizeof(uint32_t), st) != cudaSuccess)
+    return -1;
   if (M.n == 0) return 0;
   const int64_t blocks = ((M.n + 1) / 2 + 255) / 256;
-  k_tilebin_build<<<(unsigned int)blocks, 256, 0, st>>>(P, M, T, count, rec);
+  k_tilebin_build<<<(unsigned int)blocks, 256, 0, st>>>(P, M, T, count, rec, base);
   return 1;
 }
 

@@ -163,24 +163,38 @@ def test_cfg4_presorted_whole_grid(cfg4_case):
     _conservation(cfg, m, rho, jpar)
 
 
-def test_deposit_host_sliced_pipeline():
-    """orb_deposit_host above 2^22 markers: host->device copies in slices overlapped with binning
-    and deposition of the previous slice; result and point count must not depend on the slicing."""
+@pytest.mark.parametrize("adaptive", [True, False])
+def test_deposit_host_sliced_pipeline(adaptive):
+    """orb_deposit_host above 2^22 markers: the host->device copies travel in slices, each slice is
+    appended to the slack tile bins when it lands, and the deposit kernel runs once per group of
+    slices (per slice for the algorithms that read the bound arrays).  Result and point count must
+    not depend on the slicing: adaptive N_L (block-per-tile kernel), fixed N_L = 4 (persistent
+    kernel), and the global-atomics algorithm, against the oracle on all markers."""
     import dataclasses
     cfg = dataclasses.replace(W.scaled(W.CONFIGS["cfg4"], (1 << 22) + 12_345), ns=64, ntheta=128,
                               nphi=32, rho_star=1 / 120.0)
+    if not adaptive:
+        cfg = dataclasses.replace(cfg, adaptive=False, n_fixed=4)
     m = W.generate(cfg)
     rho_o, jpar_o, npts_o, _ = O.deposit_ranges(oracle_geom(cfg), oracle_policy(cfg),
                                                 *(m[f] for f in W.FIELDS), current=True)
     g = B.grid_for(cfg)
     rho = np.empty((cfg.ns + 3, cfg.ntheta, cfg.nphi))
     jpar = np.empty_like(rho)
-    for _ in range(2):      # second call reuses streams, events and scratch
+    for flags in (0, 0, B.ORB_DEPOSIT_ALGO_ATOMIC, 0):   # repeated calls reuse streams and scratch
+        rho.fill(np.nan)
+        jpar.fill(np.nan)
         npts, up, down = g.deposit_host(m["s"], m["theta"], m["phi"], m["vpar"], m["mu"], m["w"],
-                                        rho, jpar, B.policy_for(cfg))
+                                        rho, jpar, B.policy_for(cfg, flags=flags))
         assert npts == npts_o and up == 6 * 8 * cfg.n_markers and down == 2 * rho.nbytes
         assert rel_err(rho, rho_o) <= TOL
         assert rel_err(jpar, jpar_o) <= TOL
+    # the handle stays bound to the library's device copy: a device-side deposit gives the same
+    import torch
+    rho_d = torch.zeros(rho.shape, dtype=torch.float64, device="cuda")
+    g.deposit(rho_d, None, B.policy_for(cfg, flags=B.ORB_DEPOSIT_ZERO_FIRST))
+    torch.cuda.synchronize()
+    assert rel_err(rho_d.cpu().numpy(), rho_o) <= TOL
     g.destroy()
 
 
