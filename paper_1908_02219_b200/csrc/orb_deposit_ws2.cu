@@ -133,7 +133,11 @@ struct Shape {
   static constexpr int kPad = kMCap;                   // dummy entries that pad cells to batches of 4
   static constexpr int kSlots = kPts + kPad;
   static constexpr int kChan = 4 * G;                  // channels per node / marker
-  static_assert(kSlots % 4 == 0 && kPts < 65535 && kMCap < 65535, "perm entries are 16 + 16 bits");
+  // a permutation entry holds two BYTE offsets: of the point record (16 bytes each) in the low
+  // half, of the marker's channel row (kChan doubles each) in the high half
+  static constexpr unsigned kDummy = (unsigned)(kPts * 16) | ((unsigned)(kMCap * kChan * 8) << 16);
+  static_assert(kSlots % 4 == 0 && kPts * 16 < 65536 && kMCap * kChan * 8 < 65536,
+                "perm entries are 16 + 16 bits");
 };
 
 struct StageInfo {
@@ -174,7 +178,7 @@ __device__ __noinline__ void deposit_point_cell(const Params& P, int ci, double 
   for (int a = 0; a < 4; ++a) {
 #pragma unroll
     for (int b = 0; b < 4; ++b) {
-      const double v = ws[a] * wt[b];
+      const double v = ws[a] * (6.0 * wt[b]);   // chan carries 1/6 (see the producer)
       const int64_t row = ((int64_t)(ci + a) * P.nth + wrap_index(cj - 1 + b, P.nth)) * (int64_t)P.nph;
 #pragma unroll
       for (int d = 0; d < 4; ++d) {
@@ -274,7 +278,8 @@ __device__ __forceinline__ void producer(Smem<G>& S, const Params& P, const Mark
         const GuidingCentre g = guiding_centre(P, m.s, m.th, m.mu);
         const int un = g.n;
         my_points += (unsigned)un;
-        const double c = P.q * m.w * __drcp_rn((double)un);
+        // (1/6: the consumers evaluate 6 x the theta* pieces)
+        const double c = P.q * m.w * __drcp_rn((double)un) * (1.0 / 6.0);
         double wp[4];
         const int k0 = periodic_weights(wrap_2pi(m.ph), P.nph_scale, P.nph, wp);
         const bool k_ok = (k0 == k - 1);
@@ -411,7 +416,7 @@ __device__ __forceinline__ void producer(Smem<G>& S, const Params& P, const Mark
 
       // -------------------------------------------------- phase D: permutation entries, by cell
       {
-        constexpr unsigned kDummy = (unsigned)Sh::kPts | ((unsigned)Sh::kMCap << 16);
+        constexpr unsigned kDummy = Sh::kDummy;
         const unsigned int n_q = n_here * kPPL;
         for (unsigned int q = (unsigned)tid; q < n_q; q += Sh::kProd) {
           const unsigned int mt = S.meta[q];
@@ -429,7 +434,7 @@ __device__ __forceinline__ void producer(Smem<G>& S, const Params& P, const Mark
             continue;
           }
           unsigned int p = (pk & 0xffffu) + rank;
-          St.perm[p] = q | (u << 16);
+          St.perm[p] = (q << 4) | ((u * (unsigned)(kChan * 8)) << 16);
           if (rank + 1 == cnt)   // the cell's last point pads the cell to a batch of 4
             for (++p; (p & 3u) != 0; ++p) St.perm[p] = kDummy;
         }
@@ -480,7 +485,9 @@ __device__ __forceinline__ void consumer(Smem<G>& S, const Params& P, double* __
     if (n_items < 0) break;
     const int last = St.info.last, tk = St.info.k, row_base = St.info.row_base,
               cellcol_base = St.info.cellcol_base;
-    const double* mt_l = St.mtab + (G == 2 ? g : (g & 3));   // this lane's channel of a marker
+    // this lane's channel of a marker, and the point records, as byte pointers (see Shape::kDummy)
+    const char* mt_b = reinterpret_cast<const char*>(St.mtab + (G == 2 ? g : (g & 3)));
+    const char* rec_b = reinterpret_cast<const char*>(St.rec);
     const unsigned int* perm_l = St.perm + kk;               // this lane's point of a batch
 
     for (;;) {
@@ -510,16 +517,18 @@ __device__ __forceinline__ void consumer(Smem<G>& S, const Params& P, double* __
       double Ab = 0.0, Bb = 0.0;
       unsigned int pe;
 #define ORB_LD(S, e)                                                                  \
-      S##t = St.rec[(e) & 0xffffu];                                                   \
-      if (G == 2 || g < 4) S##b = mt_l[((e) >> 16) * kChan];
-      // y = t or 1 - t; the two pieces of this lane's slots are y^3/6 and 2/3 - y^2 + y^3/2
+      S##t = *reinterpret_cast<const double2*>(rec_b + ((e) & 0xffffu));              \
+      if (G == 2 || g < 4) S##b = *reinterpret_cast<const double*>(mt_b + ((e) >> 16));
+      // y = t or 1 - t; the two pieces of this lane's slots are y^3/6 and 2/3 - y^2 + y^3/2, here
+      // times 6 (y^3 and 4 - 6 y^2 + 3 y^3: the coefficients are instruction immediates); the
+      // producer folds the 1/6 into the marker's channel values
 #define ORB_MMA(S)                                                                    \
       {                                                                               \
         const double ws = fma(fma(fma(r3, S##t.x, r2), S##t.x, r1), S##t.x, r0);      \
-        const double y = y_is_t ? S##t.y : 1.0 - S##t.y;                              \
-        const double y2 = y * y;                                                      \
-        const double outer = y2 * y * (1.0 / 6.0);                                    \
-        const double mid = fma(y2, fma(0.5, y, -1.0), 2.0 / 3.0);                     \
+        const double ym = S##t.y - yoff;            /* y = |ym| */                    \
+        const double y2 = ym * ym;                                                    \
+        const double outer = y2 * fabs(ym);                                           \
+        const double mid = fma(3.0 * y2, fabs(ym) - 2.0, 4.0);                        \
         const double a0 = ws * (outer_first ? outer : mid);                           \
         const double a1 = ws * (outer_first ? mid : outer);                           \
         dmma884(c0a, c0b, a0, S##b);                                                  \
@@ -548,7 +557,7 @@ __device__ __forceinline__ void consumer(Smem<G>& S, const Params& P, double* __
         int nb = (int)(((pk >> 16) + 3u) >> 2);                                       \
         pk = St.cs[c_first + cc + (U) + 1];                                           \
         const int b0 = (hi - (U)) & 3;                                                \
-        const bool y_is_t = (b0 & 1) != 0;                                            \
+        const double yoff = ((U) & 1) ? yoff_odd : yoff_even;                         \
         const bool outer_first = b0 == 0 || b0 == 3;                                  \
         _Pragma("unroll 1") for (; nb >= 2; nb -= 2) {                                \
           ORB_LD(B, pe)                                                               \
@@ -569,6 +578,8 @@ __device__ __forceinline__ void consumer(Smem<G>& S, const Params& P, double* __
         ORB_PARK(U)                                                                   \
       }
 
+      // y = |t - yoff|: t for the odd pieces, 1 - t for the even ones (b0 = (hi - U) & 3)
+      const double yoff_even = hi ? 0.0 : 1.0, yoff_odd = 1.0 - yoff_even;
       // parked columns: pair i holds node columns 4i + hi (first slot) and 4i + hi + 2 (second)
       double q0a[4], q0b[4], q1a[4], q1b[4];
       double t0a = 0.0, t0b = 0.0, t1a = 0.0, t1b = 0.0;
@@ -684,7 +695,7 @@ k_deposit_ws2(const Params P, const Markers M, const uint32_t* __restrict__ cell
   for (int x = tid; x < kNH * kNW * Sh::kChan; x += Sh::kThreads) S.tile[x] = 0.0;
   for (int x = tid; x < kCells; x += Sh::kThreads) S.count[x] = 0;
   for (int s = 0; s < kStages; ++s) {
-    constexpr unsigned kDummy = (unsigned)Sh::kPts | ((unsigned)Sh::kMCap << 16);
+    constexpr unsigned kDummy = Sh::kDummy;
     for (int x = tid; x < Sh::kSlots + 16; x += Sh::kThreads) S.st[s].perm[x] = kDummy;
     if (tid < Sh::kChan) S.st[s].mtab[Sh::kMCap * Sh::kChan + tid] = 0.0;   // the zero marker
     if (tid == 0) S.st[s].rec[Sh::kPts] = make_double2(0.0, 0.0);           // the dummy point
