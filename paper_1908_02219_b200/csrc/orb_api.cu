@@ -538,7 +538,7 @@ int orb_deposit(orb_grid_t* g, double* rho, double* jpar, const orb_nl_policy_t*
     // persistent kernel are faster there (single_node electrons: 2.65 vs 3.19 ms)
     l = launch_deposit_ws(P, M, g->bin.cell_start, TB, rho, jpar, g->d_points, g->sms, st);
   } else {
-    // fixed N_L = 2..4: the persistent kernel with whole-tile-sized chunks (cfg3 15.1 vs 16.4 ms,
+    // fixed N_L = 2..4: the persistent kernel with whole-tile-sized chunks (cfg3 14.4 vs 16.4 ms,
     // cfg1 2.9 vs 3.6 ms against ORB_DEPOSIT_ALGO_TILE_WS)
     l = launch_deposit_ws2(P, M, g->bin.cell_start, TB, rho, jpar, g->d_points, g->sms, st);
   }

@@ -11,7 +11,8 @@
 // (t_s, t_theta): one radial cubic with lane-constant coefficients (tabulated pieces of the clamped
 // basis) and the two cardinal theta* pieces of its accumulator slots, y^3/6 and 2/3 - y^2 + y^3/2 at
 // y = t or 1 - t.  A stage of 384 markers (rho + j_par; 512 for rho only) is 58 KB, so three
-// stages fit.  Measured (cfg3 / cfg1): 15.1 / 2.9 ms against 16.4 / 3.6 ms for v5.  The chunk
+// stages fit.  Measured (cfg3 / cfg1): 14.4 / 2.9 ms against 16.4 / 3.6 ms for v5 (15.1 ms before
+// the consumers' operand evaluation was trimmed to 53 instructions per pair of batches).  The chunk
 // capacity was swept: 256 -> 16.6 ms, 320 -> 17.0, 384 -> 15.4 (two stages; 15.1 with three),
 // 448 -> 15.7, 576 (a cfg3 tile in ONE chunk) -> 17.7: two unequal chunks per tile pipeline better
 // than one (the consumers' flush then falls on a short chunk) and better than two equal ones.
