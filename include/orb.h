@@ -317,6 +317,36 @@ int orb_spline_table_radial(int32_t ns, double *out);
  * bench.py reports `roofline_alu` against.  Synchronous; takes a few milliseconds. */
 int orb_probe_dfma(int32_t device, double *tflops);
 
+/* ---- Allocation-free deposit, for callers that cannot call cudaMalloc at all (code under CUDA
+ * graph capture, tight serving loops, harnesses that forbid it) and so cannot hold an orb_grid_t.
+ * The definition of orb_deposit (same ring, map, splines and N_L policy),
+ * computed by a variant of the one-thread-per-marker global-atomics kernel whose scratch (Larmor
+ * ring table, radial spline pieces, point counter) lives in ONE file-scope device array of
+ * 139 776 bytes (csrc/orb_noalloc.cu) that every GPU loading the library holds until exit.
+ * Limit: desc->ns <= ORB_NOALLOC_MAX_NS, else ORB_E_INVAL with the reason in errbuf; the marker
+ * count is not limited.  The call makes no cudaMalloc / cudaFree and calls no allocating routine:
+ * it clears the counter, rebuilds both tables on the device for this call's (ns, alpha0), and
+ * launches the deposit, all on `stream`.
+ *   desc                 grid, geometry, species, device (as for orb_grid_create; only read)
+ *   n; s .. w            DEVICE marker arrays of n doubles, 16-byte aligned, only read; vpar may
+ *                        be NULL iff jpar is NULL
+ *   rho, jpar            DEVICE grids of (ns + 3) * ntheta * nphi doubles (layout of
+ *                        orb_grid_shape), 16-byte aligned, ADDED to; jpar may be NULL
+ *   policy               N_L policy; of the flags only ORB_DEPOSIT_ZERO_FIRST is accepted
+ *   n_points             NULL: the call is asynchronous.  Otherwise (HOST pointer) the call waits
+ *                        for `stream` and returns the sum of N_L (not under graph capture)
+ *   errbuf, errbuf_len   optional HOST buffer that receives the message of a failing call
+ * All calls on a device SHARE the scratch array, which keeps the last call's contents: calls on
+ * one stream are ordered and safe; calls that overlap on the GPU (other streams, concurrently
+ * replayed graphs) race on it and must be serialised by the caller.
+ * Speed: that of ORB_DEPOSIT_ALGO_ATOMIC (about 10x slower than the tile kernels on cfg3). */
+#define ORB_NOALLOC_MAX_NS 1024
+int orb_deposit_noalloc(const orb_grid_desc_t *desc, int64_t n, const double *s,
+                        const double *theta, const double *phi, const double *vpar,
+                        const double *mu, const double *w, double *rho, double *jpar,
+                        const orb_nl_policy_t *policy, void *stream, int64_t *n_points,
+                        char *errbuf, int32_t errbuf_len);
+
 /* ------------------------------------------------------------------------------------------ */
 
 /* Static text for a status code. */

@@ -24,12 +24,13 @@ ORB_MARKERS_SORTED = 0x1
 ORB_MARKERS_TILE_BINS = 0x2
 ORB_MAX_NL = 32
 ORB_MAX_FIELDS = 8
+ORB_NOALLOC_MAX_NS = 1024
 
 # every symbol include/orb.h declares
 SYMBOLS = ("orb_grid_create", "orb_grid_destroy", "orb_grid_shape", "orb_markers_bind",
            "orb_reserve", "orb_ring_reserve", "orb_markers_bin", "orb_markers_refresh", "orb_markers_rebin", "orb_last_moved",
            "orb_markers_layout", "orb_debug_tilebins", "orb_deposit", "orb_gather", "orb_grid_zero", "orb_last_points", "orb_last_fallback_points", "orb_deposit_host",
-           "orb_launch_count", "orb_debug_counters", "orb_debug_binned", "orb_probe_dfma", "orb_spline_table_radial", "orb_strerror", "orb_last_error", "orb_version")
+           "orb_launch_count", "orb_debug_counters", "orb_debug_binned", "orb_probe_dfma", "orb_deposit_noalloc", "orb_spline_table_radial", "orb_strerror", "orb_last_error", "orb_version")
 
 
 class OrbError(RuntimeError):
@@ -90,6 +91,8 @@ def lib():
     L.orb_deposit_host.argtypes = [vp, C.c_int64, dp, dp, dp, dp, dp, dp, dp, dp,
                                    C.POINTER(NlPolicy), i64p, i64p, i64p]
     L.orb_launch_count.argtypes = [vp, i64p]
+    L.orb_deposit_noalloc.argtypes = [C.POINTER(GridDesc), C.c_int64, dp, dp, dp, dp, dp, dp, dp, dp,
+                                      C.POINTER(NlPolicy), vp, i64p, C.c_char_p, C.c_int32]
     L.orb_debug_binned.argtypes = [vp, dp, dp, C.POINTER(C.c_int32)]
     L.orb_spline_table_radial.argtypes = [C.c_int32, dp]
     L.orb_strerror.argtypes = [C.c_int]
@@ -140,6 +143,23 @@ def spline_table_radial(ns: int):
     out = np.empty((ns, 4, 4), dtype=np.float64)
     _check(lib().orb_spline_table_radial(ns, out.ctypes.data))
     return out
+
+
+def deposit_noalloc(desc: GridDesc, s, theta, phi, vpar, mu, w, rho, jpar, pol: NlPolicy,
+                    stream=None, n=None, want_points=False):
+    """orb_deposit_noalloc: handle-free deposit that allocates nothing (static device scratch,
+    ns <= ORB_NOALLOC_MAX_NS).  Device arrays in, device grids added to.  Returns the sum of N_L
+    if want_points (the call then waits for the stream), else None (asynchronous)."""
+    if n is None:
+        n = s.numel() if hasattr(s, "numel") else len(s)
+    err = C.create_string_buffer(512)
+    pts = C.c_int64(0)
+    code = lib().orb_deposit_noalloc(C.byref(desc), n, _ptr(s), _ptr(theta), _ptr(phi), _ptr(vpar),
+                                     _ptr(mu), _ptr(w), _ptr(rho), _ptr(jpar), C.byref(pol), stream,
+                                     C.byref(pts) if want_points else None, err, len(err))
+    if code != ORB_OK:
+        raise OrbError(code, err.value.decode() or lib().orb_strerror(code).decode())
+    return pts.value if want_points else None
 
 
 class Grid:
