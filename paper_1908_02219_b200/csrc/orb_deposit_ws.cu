@@ -229,15 +229,16 @@ __device__ __forceinline__ void producer(Smem<G, PW, CW>& S, const Params& P, co
     }
   };
   // marker v of the tile -> global marker index (lanes hold the descriptor rows)
+  // (binary search for the last run whose offset is <= v: empty runs share their offset with the
+  // next one, so the run found is the one that holds v; -1 beyond the tile's last marker)
   auto marker_index = [&](uint32_t v, uint32_t rb, uint32_t rn, uint32_t ro) -> int64_t {
-    int64_t p = -1;
-#pragma unroll
-    for (int r = 0; r < kTileI; ++r) {
-      const uint32_t b = __shfl_sync(kFull, rb, r), n = __shfl_sync(kFull, rn, r),
-                     o = __shfl_sync(kFull, ro, r);
-      if (v >= o && v - o < n) p = (int64_t)b + (v - o);
-    }
-    return p;
+    static_assert(kTileI == 8, "three search steps");
+    int r = (v >= __shfl_sync(kFull, ro, 4)) ? 4 : 0;
+    r += (v >= __shfl_sync(kFull, ro, r + 2)) ? 2 : 0;
+    r += (v >= __shfl_sync(kFull, ro, r + 1)) ? 1 : 0;
+    const uint32_t o = __shfl_sync(kFull, ro, r), n = __shfl_sync(kFull, rn, r);
+    const int64_t p = (int64_t)__shfl_sync(kFull, rb, r) + (v - o);
+    return (v - o < n) ? p : -1;
   };
 
   uint32_t nb_rb, nb_rn;       // next tile's descriptor (prefetched)
