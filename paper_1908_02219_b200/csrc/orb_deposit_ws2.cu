@@ -656,22 +656,29 @@ __device__ __forceinline__ void consumer(Smem<G>& S, const Params& P, double* __
     ORB_CLK(ctid == 0, 9);
 
     if (last) {
-      // a9: all consumers are done with the tile -> flush it once and clear it.  kChan consecutive
-      // lanes run along the channels of a node (4 phi planes = one 32-byte sector per grid).
+      // a9: all consumers are done with the tile -> flush it once and clear it.  kChan / 2
+      // consecutive lanes run along the channels of a node (4 phi planes = one 32-byte sector per
+      // grid); one thread = two channels (two consecutive phi planes): 128-bit shared loads and
+      // clears, the node's index arithmetic once per pair.
       named_bar_sync(2, Sh::kCons);
-      const int ch = ctid % kChan;
-      double* __restrict__ out = ((G == 2 && ch >= 4) ? jpar : rho) + wrap_index(tk - 1 + (ch & 3), P.nph);
+      constexpr int kPairs = kChan / 2;
+      const int ch = 2 * (ctid % kPairs);
+      double* __restrict__ out = (G == 2 && ch >= 4) ? jpar : rho;
+      const int ka = wrap_index(tk - 1 + (ch & 3), P.nph), kb = wrap_index(tk + (ch & 3), P.nph);
       const int64_t row_stride = (int64_t)P.nth * P.nph;
-      for (int node = ctid / kChan; node < kNH * kNW; node += Sh::kCons / kChan) {
-        const double v = S.tile[node * kChan + ch];
-        if (v == 0.0) continue;
-        S.tile[node * kChan + ch] = 0.0;
+      for (int node = ctid / kPairs; node < kNH * kNW; node += Sh::kCons / kPairs) {
+        double2* cell = reinterpret_cast<double2*>(S.tile + node * kChan + ch);
+        const double2 v = *cell;
+        if (v.x == 0.0 && v.y == 0.0) continue;
+        *cell = make_double2(0.0, 0.0);
         const int nr = node / kNW, tc = node - nr * kNW;
         const int gi = row_base + nr;           // zero outside [0, ns + 2]: no point maps there
         int gj = cellcol_base - 1 + tc;
         while (gj < 0) gj += P.nth;
         while (gj >= P.nth) gj -= P.nth;
-        atomicAdd(out + gi * row_stride + (int64_t)gj * P.nph, v);
+        double* dst = out + gi * row_stride + (int64_t)gj * P.nph;
+        if (v.x != 0.0) atomicAdd(dst + ka, v.x);
+        if (v.y != 0.0) atomicAdd(dst + kb, v.y);
       }
       named_bar_sync(2, Sh::kCons);
       ORB_CLK(ctid == 0, 10);
